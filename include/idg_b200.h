@@ -1,0 +1,182 @@
+/* idg_b200.h -- C ABI of the B200-native image-domain-gridding (IDG) hot path.
+ *
+ * Method: arxiv 2502.17789 (Hodgson 2025, "That pesky A-term", the Pigi imager); citations
+ * are "PAPER.md:<line>" of the paper text plus the section / equation they fall in.
+ * "R<n>" are the readings of silent or ambiguous points listed in DESIGN.md.
+ *
+ * Path (§2.5 :152-174):
+ *   imaging    : gridder (Eq. 10 :133-137) -> A-term sandwich + taper (:156, §3.3 :251-257)
+ *                -> subgrid FFT (:157) -> adder (Eq. 6 :102, :158)
+ *   prediction : splitter (:169) -> inverse subgrid FFT (:170) -> taper + A-term (Eq. 13 :173)
+ *                -> degridder (Eq. 13 :171-174)
+ *
+ * Conventions:
+ *   Ng grid size (even), cell [rad], S = Ng*cell; L subgrid size in {32,64,96,128}; P total
+ *   kernel padding in pixels; kappa_c = nu_c / 299792458.0; row r = b*n_times + t
+ *   (baseline-major); u = u_m(r)*kappa_c [wavelengths].
+ *   subgrid s = (b, t0, nt, c0, nc, x0, y0, wl): rows b*n_times + t0 .. +nt, channels c0 .. +nc,
+ *   lower-left master-grid pixel (x0, y0), w-layer wl (signed).  Centre cx = x0 + L/2,
+ *   u0 = (cx - Ng/2)/S, v0 likewise, w0 = (wl + 1/2)*w_step if w_step > 0 else 0.
+ *   subgrid pixel (y, x): l = (x - L/2)*S/L, m = (y - L/2)*S/L, n' = sqrt(1-l^2-m^2) - 1.
+ *   phase [cycles] phi = (u-u0) l + (v-v0) m + (w-w0) n'.
+ *   2x2 matrices are row-major: vis[r, c, 0..3] = (XX, XY, YX, YY); Jones M[st, it, y, x, 2, 2].
+ *
+ * All *_dev pointers are caller-owned device memory (16-byte aligned); all *_host pointers are
+ * caller-owned host memory.  The library allocates on the device only the plan metadata it
+ * uploads on first use (freed by idg_plan_destroy).  All device work is enqueued on the
+ * caller's stream (a cudaStream_t passed as void*; NULL = default stream) and the calls return
+ * without synchronising unless stated.  Every function returns 0 on success or a negative
+ * IDG_E* code; idg_last_error() gives a thread-local message.  There is no CPU fallback: a
+ * device call on a machine without a usable sm_100 GPU returns IDG_ECUDA.
+ */
+#ifndef IDG_B200_H
+#define IDG_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define IDG_API __attribute__((visibility("default")))
+#else
+#define IDG_API
+#endif
+
+#define IDG_OK            0
+#define IDG_EINVAL       -1   /* bad argument (null pointer, non-ascending channels, bad sizes)  */
+#define IDG_EUNSUPPORTED -2   /* subgrid size not in {32,64,96,128}                              */
+#define IDG_ENOMEM       -3   /* workspace too small / host allocation failed                   */
+#define IDG_ECUDA        -4   /* CUDA runtime error (message in idg_last_error)                 */
+
+#define IDG_GRID   0          /* direction selectors for idg_workspace_bytes                    */
+#define IDG_DEGRID 1
+
+/* stage selectors for idg_grid_subgrids */
+#define IDG_STAGE_GRIDDER 0   /* after gridder + A-term + taper (steps a1-a3), image domain     */
+#define IDG_STAGE_FFT     1   /* after the subgrid FFT (step a4), uv domain                     */
+
+typedef struct idg_plan idg_plan;          /* opaque; host-owned; immutable after create          */
+
+typedef struct {
+  int32_t grid_size;      /* Ng, even                                                            */
+  int32_t subgrid_size;   /* L in {32, 64, 96, 128}                                              */
+  int32_t padding;        /* P, total kernel padding in pixels, 0 <= P < L-1  (R8)               */
+  int32_t n_stations;
+  int32_t n_baselines;
+  int32_t n_times;
+  int32_t n_chan;
+  int32_t aterm_period;   /* timesteps per A-term interval, >= 1 (R6)                            */
+  double  cell_size;      /* rad                                                                 */
+  double  w_step;         /* wavelengths; 0 => single layer with w0 = 0 (R9)                     */
+  double  comfort;        /* fraction of the usable span a channel range may fill (R7); 0.75     */
+  int64_t max_batch_subgrids; /* subgrids processed per batch (§3.4 :259-267, R18);
+                                 0 => library default                                            */
+} idg_params;
+
+/* ---- planner: visibility table -> subgrids (§2.2 :62-72, §2.4 :141-143, §3.1
+ * :186-200, §3.3 :255; the deterministic reading is DESIGN.md "O1").  Host only: works on a
+ * machine without a GPU.
+ *   uvw_m_host     [n_baselines*n_times, 3] float64 metres, row r = b*n_times + t
+ *   freqs_host     [n_chan] float64 Hz, strictly ascending (R11) else IDG_EINVAL
+ *   baselines_host [n_baselines, 2] int32 station pairs (p, q)
+ * The plan keeps its own copies; the inputs may be freed after the call. */
+IDG_API int  idg_plan_create(const idg_params* params, const double* uvw_m_host, const double* freqs_host,
+                     const int32_t* baselines_host, idg_plan** out);
+IDG_API void idg_plan_destroy(idg_plan* plan);
+
+/* Counts: subgrids, number of w-layers W = wl_max - wl_min + 1 (1 if no subgrids), wl_min,
+ * visibilities covered by a subgrid and visibilities dropped because their subgrid would
+ * leave the master grid.  Any output pointer may be NULL. */
+IDG_API int  idg_plan_counts(const idg_plan* plan, int64_t* n_subgrids, int32_t* n_wlayers, int32_t* wl_min,
+                     int64_t* n_vis_planned, int64_t* n_vis_dropped);
+
+/* sub_host [n_subgrids, 8] int32 rows (b, t0, nt, c0, nc, x0, y0, wl), sorted by (wl, b, t0, c0). */
+IDG_API int  idg_plan_export(const idg_plan* plan, int32_t* sub_host);
+
+/* Bytes of device workspace idg_grid / idg_degrid need (the subgrid stack of one batch,
+ * PAPER.md:210 "a contiguous stack of L x L arrays"). */
+IDG_API size_t idg_workspace_bytes(const idg_plan* plan, int direction);
+
+/* ---- imaging direction, steps 2.i-2.iii of PAPER.md:155-158 over all subgrids of the plan.
+ *   vis_dev    [n_rows, n_chan, 4] complex64 (interleaved re, im)
+ *   aterms_dev [n_stations, n_intervals, L, L, 2, 2] complex64, n_intervals = ceil(n_times/aterm_period);
+ *              applied as M_p X M_q^H (R5): pass A^-1 for paper-style imaging (Eq. 10)
+ *   taper_dev  [L, L] float32 (R4, R15)
+ *   grid_dev   [n_wlayers, 4, Ng, Ng] complex64, ACCUMULATED INTO (caller zeroes)
+ * The adder is atomic-free and its summation order is fixed: results are bitwise reproducible. */
+IDG_API int  idg_grid(const idg_plan* plan, const void* vis_dev, const void* aterms_dev, const float* taper_dev,
+              void* grid_dev, void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
+
+/* ---- prediction direction, steps 3.i-3.iii of PAPER.md:168-174.  Writes vis_dev[r, c, :]
+ * for every visibility covered by a subgrid and leaves the others untouched.  The same taper
+ * array multiplies (R4) and the same sandwich M_p X M_q^H is applied (R5: pass A). */
+IDG_API int  idg_degrid(const idg_plan* plan, const void* grid_dev, const void* aterms_dev, const float* taper_dev,
+                void* vis_dev, void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
+
+/* ---- the same two calls on HOST buffers (pinned memory recommended).  They copy the inputs
+ * to `arena_dev`, run the device path on `cuda_stream`, copy the result back (grid_host is
+ * accumulated into: it is uploaded first) and synchronise the stream before returning.
+ * arena_dev must hold idg_host_arena_bytes(plan, direction) bytes. */
+IDG_API size_t idg_host_arena_bytes(const idg_plan* plan, int direction);
+IDG_API int  idg_grid_host(const idg_plan* plan, const void* vis_host, const void* aterms_host,
+                   const float* taper_host, void* grid_host, void* arena_dev, size_t arena_bytes,
+                   void* cuda_stream);
+IDG_API int  idg_degrid_host(const idg_plan* plan, const void* grid_host, const void* aterms_host,
+                     const float* taper_host, void* vis_host, void* arena_dev, size_t arena_bytes,
+                     void* cuda_stream);
+
+/* ---- stage-level entry points (used by the parity tests; same kernels as above) ----------- */
+
+/* Subgrids [first, first+count) through the gridder (+A-term+taper) and, if stage ==
+ * IDG_STAGE_FFT, the subgrid FFT.  subgrids_dev [count, 4, L, L] complex64 (pol-major planes). */
+IDG_API int  idg_grid_subgrids(const idg_plan* plan, int64_t first, int64_t count, const void* vis_dev,
+                       const void* aterms_dev, const float* taper_dev, void* subgrids_dev,
+                       int stage, void* cuda_stream);
+
+/* Image-domain subgrids [first, first+count) (after the inverse FFT, before taper / A-term)
+ * through taper + A-term + degridder into vis_dev. */
+IDG_API int  idg_degrid_subgrids(const idg_plan* plan, int64_t first, int64_t count, const void* subgrids_dev,
+                         const void* aterms_dev, const float* taper_dev, void* vis_dev,
+                         void* cuda_stream);
+
+/* Centred L x L DFT of `n_planes` planes in place, each scaled by 1/L^2 (R1, R2):
+ * direction +1: out[gy,gx] = L^-2 sum in[y,x] exp(-2 pi i((gy-L/2)(y-L/2)+(gx-L/2)(x-L/2))/L)
+ * direction -1: the same with exp(+...)  (Eq. 7-8 :107-117). */
+IDG_API int  idg_subgrid_fft(int32_t subgrid_size, int64_t n_planes, void* planes_dev, int direction,
+                     void* cuda_stream);
+
+/* Adder / splitter for subgrids [first, first+count) (Eq. 6 :102, :158, :169):
+ *   adder   : grid[wl - wl_min, pol, y0+gy, x0+gx] += subgrids[s - first, pol, gy, gx]
+ *   splitter: subgrids[s - first, pol, gy, gx]      = grid[wl - wl_min, pol, y0+gy, x0+gx]   */
+IDG_API int  idg_adder(const idg_plan* plan, int64_t first, int64_t count, const void* subgrids_dev,
+               void* grid_dev, void* cuda_stream);
+IDG_API int  idg_splitter(const idg_plan* plan, int64_t first, int64_t count, const void* grid_dev,
+                  void* subgrids_dev, void* cuda_stream);
+
+/* ---- per-kernel timing (CUDA events recorded on the caller's stream around every kernel
+ * launch while enabled; off by default).  idg_profile_read waits for the recorded events,
+ * adds their durations into ms_out[kind] / launches_out[kind] (kind = IDG_K_*, arrays of
+ * IDG_K_COUNT) and clears the record. */
+#define IDG_K_GRIDDER   0
+#define IDG_K_FFT       1
+#define IDG_K_ADDER     2
+#define IDG_K_SPLITTER  3
+#define IDG_K_IFFT      4
+#define IDG_K_DEGRIDDER 5
+#define IDG_K_COUNT     6
+IDG_API int  idg_profile_enable(int on);
+IDG_API int  idg_profile_read(double* ms_out, int64_t* launches_out);
+
+/* Number of kernels the library has launched in this process (for bench.py's gpu_launches). */
+IDG_API int64_t idg_launch_count(void);
+
+IDG_API const char* idg_last_error(void);
+IDG_API const char* idg_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* IDG_B200_H */

@@ -1,0 +1,283 @@
+"""Thin Python binding over the C-ABI library `libidg_b200.so` (include/idg_b200.h).
+
+Argument marshalling only: every step of the IDG hot path (§2.5 :152-174) runs in the
+CUDA kernels behind the C ABI.  PyTorch supplies device memory and streams.  The functions
+mirror the C entry points one to one (`idg_grid` -> `grid`, ...).  There is no CPU fallback: if
+the library is missing, or a device call is made without a B200, an exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libidg_b200.so")
+
+IDG_GRID, IDG_DEGRID = 0, 1
+STAGE_GRIDDER, STAGE_FFT = 0, 1
+
+# every symbol include/idg_b200.h declares
+SYMBOLS = (
+    "idg_plan_create", "idg_plan_destroy", "idg_plan_counts", "idg_plan_export", "idg_workspace_bytes",
+    "idg_grid", "idg_degrid", "idg_host_arena_bytes", "idg_grid_host", "idg_degrid_host",
+    "idg_grid_subgrids", "idg_degrid_subgrids", "idg_subgrid_fft", "idg_adder", "idg_splitter",
+    "idg_profile_enable", "idg_profile_read", "idg_launch_count", "idg_last_error", "idg_version",
+)
+KERNEL_KINDS = ("gridder", "fft", "adder", "splitter", "ifft", "degridder")
+
+
+class IdgError(RuntimeError):
+    pass
+
+
+class _Params(ctypes.Structure):
+    _fields_ = [
+        ("grid_size", ctypes.c_int32), ("subgrid_size", ctypes.c_int32), ("padding", ctypes.c_int32),
+        ("n_stations", ctypes.c_int32), ("n_baselines", ctypes.c_int32), ("n_times", ctypes.c_int32),
+        ("n_chan", ctypes.c_int32), ("aterm_period", ctypes.c_int32),
+        ("cell_size", ctypes.c_double), ("w_step", ctypes.c_double), ("comfort", ctypes.c_double),
+        ("max_batch_subgrids", ctypes.c_int64),
+    ]
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen the in-tree library; raises if it has not been built (see build.py)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise IdgError(f"{LIB_PATH} not found: build it with `python -m paper_2502_17789_b200.build` "
+                       "(there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i64, i32, sz = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_size_t
+    lib.idg_plan_create.argtypes = [ctypes.POINTER(_Params), vp, vp, vp, ctypes.POINTER(vp)]
+    lib.idg_plan_create.restype = ctypes.c_int
+    lib.idg_plan_destroy.argtypes = [vp]
+    lib.idg_plan_destroy.restype = None
+    lib.idg_plan_counts.argtypes = [vp, ctypes.POINTER(i64), ctypes.POINTER(i32), ctypes.POINTER(i32),
+                                    ctypes.POINTER(i64), ctypes.POINTER(i64)]
+    lib.idg_plan_counts.restype = ctypes.c_int
+    lib.idg_plan_export.argtypes = [vp, vp]
+    lib.idg_plan_export.restype = ctypes.c_int
+    lib.idg_workspace_bytes.argtypes = [vp, ctypes.c_int]
+    lib.idg_workspace_bytes.restype = sz
+    lib.idg_host_arena_bytes.argtypes = [vp, ctypes.c_int]
+    lib.idg_host_arena_bytes.restype = sz
+    lib.idg_grid.argtypes = [vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.idg_grid.restype = ctypes.c_int
+    lib.idg_degrid.argtypes = [vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.idg_degrid.restype = ctypes.c_int
+    lib.idg_grid_host.argtypes = [vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.idg_grid_host.restype = ctypes.c_int
+    lib.idg_degrid_host.argtypes = [vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.idg_degrid_host.restype = ctypes.c_int
+    lib.idg_grid_subgrids.argtypes = [vp, i64, i64, vp, vp, vp, vp, ctypes.c_int, vp]
+    lib.idg_grid_subgrids.restype = ctypes.c_int
+    lib.idg_degrid_subgrids.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
+    lib.idg_degrid_subgrids.restype = ctypes.c_int
+    lib.idg_subgrid_fft.argtypes = [i32, i64, vp, ctypes.c_int, vp]
+    lib.idg_subgrid_fft.restype = ctypes.c_int
+    lib.idg_adder.argtypes = [vp, i64, i64, vp, vp, vp]
+    lib.idg_adder.restype = ctypes.c_int
+    lib.idg_splitter.argtypes = [vp, i64, i64, vp, vp, vp]
+    lib.idg_splitter.restype = ctypes.c_int
+    lib.idg_profile_enable.argtypes = [ctypes.c_int]
+    lib.idg_profile_enable.restype = ctypes.c_int
+    lib.idg_profile_read.argtypes = [vp, vp]
+    lib.idg_profile_read.restype = ctypes.c_int
+    lib.idg_launch_count.argtypes = []
+    lib.idg_launch_count.restype = i64
+    lib.idg_last_error.argtypes = []
+    lib.idg_last_error.restype = ctypes.c_char_p
+    lib.idg_version.argtypes = []
+    lib.idg_version.restype = ctypes.c_char_p
+    _lib = lib
+    return lib
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != 0:
+        msg = load_library().idg_last_error().decode("utf-8", "replace")
+        raise IdgError(f"{what} failed with code {rc}: {msg}")
+
+
+def _ptr(t) -> int:
+    """Device / host pointer of a torch tensor or numpy array (contiguous)."""
+    if isinstance(t, np.ndarray):
+        if not t.flags["C_CONTIGUOUS"]:
+            raise ValueError("array must be C-contiguous")
+        return t.ctypes.data
+    if not t.is_contiguous():
+        raise ValueError("tensor must be contiguous")
+    return t.data_ptr()
+
+
+def _stream_ptr(stream) -> int | None:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def _need_cuda(*tensors) -> None:
+    for t in tensors:
+        if not getattr(t, "is_cuda", False):
+            raise IdgError("device entry points need CUDA tensors (there is no CPU fallback)")
+
+
+@dataclass(frozen=True)
+class PlanCounts:
+    n_subgrids: int
+    n_wlayers: int
+    wl_min: int
+    n_vis_planned: int
+    n_vis_dropped: int
+
+
+class Plan:
+    """Owner of an `idg_plan*` (idg_plan_create / idg_plan_destroy)."""
+
+    def __init__(self, *, grid_size, subgrid_size, padding, cell_size, w_step, n_stations, n_times, n_chan,
+                 aterm_period, uvw_m, freqs, baselines, comfort=0.75, max_batch_subgrids=0):
+        lib = load_library()
+        uvw_m = np.ascontiguousarray(uvw_m, dtype=np.float64)
+        freqs = np.ascontiguousarray(freqs, dtype=np.float64)
+        baselines = np.ascontiguousarray(baselines, dtype=np.int32)
+        n_bl = baselines.shape[0]
+        if uvw_m.shape != (n_bl * n_times, 3) or freqs.shape != (n_chan,) or baselines.shape != (n_bl, 2):
+            raise ValueError("uvw_m must be [n_bl*n_times,3], freqs [n_chan], baselines [n_bl,2]")
+        self.params = _Params(grid_size, subgrid_size, padding, n_stations, n_bl, n_times, n_chan, aterm_period,
+                              cell_size, w_step, comfort, max_batch_subgrids)
+        handle = ctypes.c_void_p()
+        _check(lib.idg_plan_create(ctypes.byref(self.params), uvw_m.ctypes.data, freqs.ctypes.data,
+                                   baselines.ctypes.data, ctypes.byref(handle)), "idg_plan_create")
+        self._h = handle
+        self.n_rows = n_bl * n_times
+        self.n_intervals = -(-n_times // aterm_period)
+
+    def __del__(self):
+        h = getattr(self, "_h", None)
+        if h and _lib is not None:
+            _lib.idg_plan_destroy(h)
+            self._h = None
+
+    @property
+    def handle(self):
+        return self._h
+
+    def counts(self) -> PlanCounts:
+        n, w, wl, pl, dr = ctypes.c_int64(), ctypes.c_int32(), ctypes.c_int32(), ctypes.c_int64(), ctypes.c_int64()
+        _check(load_library().idg_plan_counts(self._h, ctypes.byref(n), ctypes.byref(w), ctypes.byref(wl),
+                                              ctypes.byref(pl), ctypes.byref(dr)), "idg_plan_counts")
+        return PlanCounts(n.value, w.value, wl.value, pl.value, dr.value)
+
+    def export(self) -> np.ndarray:
+        n = self.counts().n_subgrids
+        sub = np.zeros((n, 8), np.int32)
+        _check(load_library().idg_plan_export(self._h, sub.ctypes.data), "idg_plan_export")
+        return sub
+
+    def workspace_bytes(self, direction=IDG_GRID) -> int:
+        return int(load_library().idg_workspace_bytes(self._h, direction))
+
+    def host_arena_bytes(self, direction=IDG_GRID) -> int:
+        return int(load_library().idg_host_arena_bytes(self._h, direction))
+
+
+def plan_from_config(cfg, uvw_m, freqs, baselines, max_batch_subgrids=0) -> Plan:
+    """Convenience: a Plan from a `synth.Config`-like object (attribute names as in include/idg_b200.h)."""
+    return Plan(grid_size=cfg.grid_size, subgrid_size=cfg.subgrid_size, padding=cfg.padding,
+                cell_size=cfg.cell_size, w_step=cfg.w_step, n_stations=cfg.n_stations, n_times=cfg.n_times,
+                n_chan=cfg.n_chan, aterm_period=cfg.aterm_period, uvw_m=uvw_m, freqs=freqs, baselines=baselines,
+                comfort=cfg.comfort, max_batch_subgrids=max_batch_subgrids)
+
+
+def grid(plan: Plan, vis, aterms, taper, grid_out, workspace, stream=None) -> None:
+    """idg_grid: accumulate all subgrids of the plan into grid_out [W,4,Ng,Ng] complex64."""
+    _need_cuda(vis, aterms, taper, grid_out, workspace)
+    _check(load_library().idg_grid(plan.handle, _ptr(vis), _ptr(aterms), _ptr(taper), _ptr(grid_out),
+                                   _ptr(workspace), workspace.numel() * workspace.element_size(),
+                                   _stream_ptr(stream)), "idg_grid")
+
+
+def degrid(plan: Plan, grid_in, aterms, taper, vis_out, workspace, stream=None) -> None:
+    """idg_degrid: predict every planned visibility into vis_out [n_rows,n_chan,4] complex64."""
+    _need_cuda(vis_out, aterms, taper, grid_in, workspace)
+    _check(load_library().idg_degrid(plan.handle, _ptr(grid_in), _ptr(aterms), _ptr(taper), _ptr(vis_out),
+                                     _ptr(workspace), workspace.numel() * workspace.element_size(),
+                                     _stream_ptr(stream)), "idg_degrid")
+
+
+def grid_host(plan: Plan, vis, aterms, taper, grid_io, arena, stream=None) -> None:
+    """idg_grid_host: host buffers in, host grid accumulated; copies run inside the call."""
+    _need_cuda(arena)
+    _check(load_library().idg_grid_host(plan.handle, _ptr(vis), _ptr(aterms), _ptr(taper), _ptr(grid_io),
+                                        _ptr(arena), arena.numel() * arena.element_size(),
+                                        _stream_ptr(stream)), "idg_grid_host")
+
+
+def degrid_host(plan: Plan, grid_in, aterms, taper, vis_io, arena, stream=None) -> None:
+    """idg_degrid_host: host buffers in, host visibilities out."""
+    _need_cuda(arena)
+    _check(load_library().idg_degrid_host(plan.handle, _ptr(grid_in), _ptr(aterms), _ptr(taper), _ptr(vis_io),
+                                          _ptr(arena), arena.numel() * arena.element_size(),
+                                          _stream_ptr(stream)), "idg_degrid_host")
+
+
+def grid_subgrids(plan: Plan, first, count, vis, aterms, taper, subgrids_out, stage=STAGE_FFT, stream=None) -> None:
+    _need_cuda(vis, aterms, taper, subgrids_out)
+    _check(load_library().idg_grid_subgrids(plan.handle, first, count, _ptr(vis), _ptr(aterms), _ptr(taper),
+                                            _ptr(subgrids_out), stage, _stream_ptr(stream)), "idg_grid_subgrids")
+
+
+def degrid_subgrids(plan: Plan, first, count, subgrids_in, aterms, taper, vis_out, stream=None) -> None:
+    _need_cuda(vis_out, aterms, taper, subgrids_in)
+    _check(load_library().idg_degrid_subgrids(plan.handle, first, count, _ptr(subgrids_in), _ptr(aterms),
+                                              _ptr(taper), _ptr(vis_out), _stream_ptr(stream)),
+           "idg_degrid_subgrids")
+
+
+def subgrid_fft(subgrid_size, planes, direction, stream=None) -> None:
+    """idg_subgrid_fft: planes [..., L, L] complex64, transformed in place."""
+    _need_cuda(planes)
+    n_planes = planes.numel() // (subgrid_size * subgrid_size)
+    _check(load_library().idg_subgrid_fft(subgrid_size, n_planes, _ptr(planes), direction, _stream_ptr(stream)),
+           "idg_subgrid_fft")
+
+
+def adder(plan: Plan, first, count, subgrids, grid_io, stream=None) -> None:
+    _need_cuda(subgrids, grid_io)
+    _check(load_library().idg_adder(plan.handle, first, count, _ptr(subgrids), _ptr(grid_io), _stream_ptr(stream)),
+           "idg_adder")
+
+
+def splitter(plan: Plan, first, count, grid_in, subgrids_out, stream=None) -> None:
+    _need_cuda(subgrids_out, grid_in)
+    _check(load_library().idg_splitter(plan.handle, first, count, _ptr(grid_in), _ptr(subgrids_out),
+                                       _stream_ptr(stream)), "idg_splitter")
+
+
+def profile_enable(on: bool) -> None:
+    _check(load_library().idg_profile_enable(1 if on else 0), "idg_profile_enable")
+
+
+def profile_read() -> dict:
+    """idg_profile_read: {kind: (milliseconds, launches)} accumulated since the last read."""
+    ms = np.zeros(len(KERNEL_KINDS), np.float64)
+    n = np.zeros(len(KERNEL_KINDS), np.int64)
+    _check(load_library().idg_profile_read(ms.ctypes.data, n.ctypes.data), "idg_profile_read")
+    return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(KERNEL_KINDS)}
+
+
+def launch_count() -> int:
+    return int(load_library().idg_launch_count())
+
+
+def version() -> str:
+    return load_library().idg_version().decode()

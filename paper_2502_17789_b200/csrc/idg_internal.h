@@ -1,0 +1,74 @@
+// Internal declarations shared by the host planner, the C-ABI layer and the kernel launchers.
+// Nothing here is visible through include/idg_b200.h.
+#pragma once
+#include <cstdint>
+#include <mutex>
+#include <string>
+#include <vector>
+
+#include "../../include/idg_b200.h"
+
+namespace idg {
+
+constexpr double kSpeedOfLight = 299792458.0;
+constexpr int kMetaStride = 12;   // int32 per subgrid on the device: b,t0,nt,c0,nc,x0,y0,wl,p,q,it,layer
+constexpr int kTile = 64;         // adder tile edge in master-grid pixels
+
+// tile -> subgrid lists for the atomic-free adder (one CSR per batch of subgrids).
+struct TileCsr {
+  std::vector<int32_t> tile_ids;   // (layer*tiles_y + ty)*tiles_x + tx of every non-empty tile
+  std::vector<int32_t> offsets;    // [n_tiles + 1] into items
+  std::vector<int32_t> items;      // subgrid indices (global), ascending within a tile
+};
+
+struct DeviceCsr {
+  int32_t* tile_ids = nullptr;
+  int32_t* offsets = nullptr;
+  int32_t* items = nullptr;
+  int32_t n_tiles = 0;
+};
+
+struct Batch {
+  int64_t first = 0, count = 0;
+  TileCsr csr;
+};
+
+struct DeviceState {
+  double* uvw = nullptr;        // [n_rows, 3] metres
+  double* kappa = nullptr;      // [n_chan] nu/c
+  int32_t* meta = nullptr;      // [n_subgrids, kMetaStride]
+  float* nprime = nullptr;      // [L, L] n'(l, m) at the subgrid pixels
+  std::vector<DeviceCsr> batch_csr;
+  int device = -1;
+};
+
+}  // namespace idg
+
+struct idg_plan {
+  idg_params par{};
+  int64_t n_rows = 0;
+  int32_t n_intervals = 0;
+  double image_size = 0.0;                // S = Ng * cell
+  std::vector<double> uvw;                // host copy [n_rows*3]
+  std::vector<double> kappa;              // nu_c / c
+  std::vector<int32_t> baselines;         // [n_bl*2]
+  std::vector<int32_t> sub;               // [n_subgrids*8]
+  int64_t n_subgrids = 0, n_vis_planned = 0, n_vis_dropped = 0;
+  int32_t wl_min = 0, n_wlayers = 1;
+  int32_t tiles_x = 0, tiles_y = 0;
+  int64_t batch_capacity = 0;             // subgrids per batch
+  std::vector<idg::Batch> batches;
+  mutable std::mutex mu;
+  mutable idg::DeviceState* dev = nullptr;   // uploaded on first device call
+};
+
+namespace idg {
+
+void set_error(const std::string& msg);
+
+// host planner (plan.cpp)
+int  plan_build(idg_plan* plan);
+void build_tile_csr(const idg_plan* plan, int64_t first, int64_t count, TileCsr* out);
+void fill_meta(const idg_plan* plan, std::vector<int32_t>* meta);
+
+}  // namespace idg

@@ -1,0 +1,49 @@
+// Launcher interface between the C-ABI layer (api.cu) and the kernels.  Plain structs of device
+// pointers and sizes; every launcher enqueues on `stream` and returns the cudaError_t of the
+// launch.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "idg_internal.h"
+
+namespace idg {
+
+struct SubgridJob {
+  const int32_t* meta;      // [n_subgrids, kMetaStride] device
+  const double* uvw;        // [n_rows, 3] metres
+  const double* kappa;      // [n_chan]
+  const float* nprime;      // [L, L] n'(l, m) at the subgrid pixels
+  const float4* aterms;     // [n_st, n_int, L, L, 2] rows of the 2x2 Jones matrices
+  const float* taper;       // [L, L]
+  int64_t first;            // first subgrid (global index)
+  int64_t count;
+  int32_t subgrid_size, grid_size, n_times, n_chan, n_intervals;
+  double image_size;        // S
+  double w_step;
+};
+
+// steps a1-a3: stage visibilities, direct sum (Eq. 10), A-term sandwich and taper.
+// out [count, 4, L, L] complex64.
+cudaError_t launch_gridder(const SubgridJob& job, const float4* vis, float2* out, cudaStream_t stream);
+
+// steps a8-a9: taper + A-term on image-domain subgrids, then the per-visibility sum (Eq. 13).
+// in [count, 4, L, L] complex64; vis [n_rows, n_chan, 4] complex64.
+cudaError_t launch_degridder(const SubgridJob& job, const float2* in, float4* vis, cudaStream_t stream);
+
+// steps a4 / a7: centred L x L DFT of n_planes planes in place, scaled by 1/L^2.
+cudaError_t launch_subgrid_fft(int L, int64_t n_planes, float2* planes, int direction, cudaStream_t stream);
+
+// step a5: tile-owner adder.  csr lists, per non-empty tile, the subgrids overlapping it.
+cudaError_t launch_adder(const int32_t* meta, const DeviceCsr& csr, int64_t first, int L, int Ng,
+                         int tiles_x, int tiles_y, const float2* subgrids, float2* grid,
+                         cudaStream_t stream);
+
+// step a6: splitter (gather).
+cudaError_t launch_splitter(const int32_t* meta, int64_t first, int64_t count, int L, int Ng,
+                            const float2* grid, float2* subgrids, cudaStream_t stream);
+
+void count_launch(int n = 1);
+
+}  // namespace idg

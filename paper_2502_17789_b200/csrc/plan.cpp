@@ -1,0 +1,197 @@
+// Host planner: visibility table -> subtables = subgrids.
+//
+// PAPER.md §2.2 :62-72 (every visibility in exactly one L x L subgrid, subgrids may overlap,
+// centre snaps to a master-grid pixel), §2.4 :141-143 (subgrids snap to a w-layer), §3.1
+// :186-200 (single pass per baseline: channel ranges that fit "comfortably", then grow in time;
+// only the corners of a subtable are tested), §3.3 :255 (one A-term interval per subgrid).
+// The deterministic reading (O1, R6-R9, R12) is restated here in C++; all arithmetic
+// is IEEE fp64 in a fixed order (this file is compiled with -ffp-contract=off) so that the plan
+// is bit-identical to the one the test oracle derives independently.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <tuple>
+
+#include "idg_internal.h"
+
+namespace idg {
+
+namespace {
+
+struct WorkItem { int32_t t0, lo, hi; };
+
+struct Emitted { int32_t v[8]; };
+
+inline bool emitted_less(const Emitted& a, const Emitted& b) {
+  // order (wl, b, t0, c0)
+  return std::make_tuple(a.v[7], a.v[0], a.v[1], a.v[3]) < std::make_tuple(b.v[7], b.v[0], b.v[1], b.v[3]);
+}
+
+}  // namespace
+
+int plan_build(idg_plan* plan) {
+  const idg_params& par = plan->par;
+  const int32_t Ng = par.grid_size, L = par.subgrid_size, P = par.padding;
+  const int32_t nT = par.n_times, nC = par.n_chan;
+  const double S = plan->image_size;
+  const double span_max = static_cast<double>(L - P - 1);
+  const double comfort_span = par.comfort * span_max;
+  const bool layered = par.w_step > 0.0;
+
+  std::vector<Emitted> out;
+  std::vector<double> X(static_cast<size_t>(nT) * nC), Y(X.size());
+  std::vector<int64_t> WL(X.size());
+  std::vector<WorkItem> work;
+  int64_t dropped = 0;
+
+  for (int32_t b = 0; b < par.n_baselines; ++b) {
+    const double* rows = plan->uvw.data() + static_cast<size_t>(b) * nT * 3;
+    for (int32_t t = 0; t < nT; ++t) {
+      const double um = rows[t * 3 + 0], vm = rows[t * 3 + 1], wm = rows[t * 3 + 2];
+      for (int32_t c = 0; c < nC; ++c) {
+        const double k = plan->kappa[c];
+        const size_t i = static_cast<size_t>(t) * nC + c;
+        X[i] = (um * k) * S;            // master-grid pixels from the centre, this exact order
+        Y[i] = (vm * k) * S;
+        WL[i] = layered ? static_cast<int64_t>(std::floor((wm * k) / par.w_step)) : 0;
+      }
+    }
+    auto at = [nC](int32_t t, int32_t c) { return static_cast<size_t>(t) * nC + c; };
+
+    for (int32_t it = 0; it < plan->n_intervals; ++it) {
+      const int32_t ta = it * par.aterm_period;
+      const int32_t tb = std::min(ta + par.aterm_period, nT);
+      work.clear();
+      work.push_back({ta, 0, nC - 1});
+      while (!work.empty()) {
+        const WorkItem w = work.back();
+        work.pop_back();
+        const int32_t t0 = w.t0, lo = w.lo, hi = w.hi;
+        const int64_t wl0 = WL[at(t0, lo)];
+        // channel range at the first timestep that fits comfortably (R7)
+        int32_t c1 = lo;
+        while (c1 + 1 <= hi &&
+               std::max(std::fabs(X[at(t0, c1 + 1)] - X[at(t0, lo)]),
+                        std::fabs(Y[at(t0, c1 + 1)] - Y[at(t0, lo)])) <= comfort_span &&
+               WL[at(t0, c1 + 1)] == wl0) {
+          ++c1;
+        }
+        if (c1 < hi) work.push_back({t0, c1 + 1, hi});
+        double xmin = std::min(X[at(t0, lo)], X[at(t0, c1)]), xmax = std::max(X[at(t0, lo)], X[at(t0, c1)]);
+        double ymin = std::min(Y[at(t0, lo)], Y[at(t0, c1)]), ymax = std::max(Y[at(t0, lo)], Y[at(t0, c1)]);
+        // grow in time while the corner bounding box still fits
+        int32_t n = 1;
+        while (t0 + n < tb) {
+          const int32_t t = t0 + n;
+          if (WL[at(t, lo)] != wl0 || WL[at(t, c1)] != wl0) break;
+          const double nxmin = std::min(xmin, std::min(X[at(t, lo)], X[at(t, c1)]));
+          const double nxmax = std::max(xmax, std::max(X[at(t, lo)], X[at(t, c1)]));
+          const double nymin = std::min(ymin, std::min(Y[at(t, lo)], Y[at(t, c1)]));
+          const double nymax = std::max(ymax, std::max(Y[at(t, lo)], Y[at(t, c1)]));
+          if ((nxmax - nxmin) > span_max || (nymax - nymin) > span_max) break;
+          xmin = nxmin; xmax = nxmax; ymin = nymin; ymax = nymax;
+          ++n;
+        }
+        if (t0 + n < tb) work.push_back({t0 + n, lo, c1});
+        // centre snaps to a master-grid pixel, round half up (R12)
+        const int64_t cx = static_cast<int64_t>(std::floor((xmin + xmax) / 2.0 + 0.5)) + Ng / 2;
+        const int64_t cy = static_cast<int64_t>(std::floor((ymin + ymax) / 2.0 + 0.5)) + Ng / 2;
+        const int64_t x0 = cx - L / 2, y0 = cy - L / 2;
+        const int32_t nc = c1 - lo + 1;
+        if (x0 < 0 || y0 < 0 || x0 + L > Ng || y0 + L > Ng) {
+          dropped += static_cast<int64_t>(n) * nc;
+          continue;
+        }
+        Emitted e;
+        e.v[0] = b; e.v[1] = t0; e.v[2] = n; e.v[3] = lo; e.v[4] = nc;
+        e.v[5] = static_cast<int32_t>(x0); e.v[6] = static_cast<int32_t>(y0);
+        e.v[7] = static_cast<int32_t>(wl0);
+        out.push_back(e);
+      }
+    }
+  }
+  std::sort(out.begin(), out.end(), emitted_less);   // keys are unique: no stability issue
+
+  plan->n_subgrids = static_cast<int64_t>(out.size());
+  plan->sub.resize(out.size() * 8);
+  int64_t planned = 0;
+  int32_t wl_lo = 0, wl_hi = 0;
+  for (size_t i = 0; i < out.size(); ++i) {
+    std::memcpy(&plan->sub[i * 8], out[i].v, sizeof(out[i].v));
+    planned += static_cast<int64_t>(out[i].v[2]) * out[i].v[4];
+    if (i == 0) { wl_lo = wl_hi = out[i].v[7]; }
+    wl_lo = std::min(wl_lo, out[i].v[7]);
+    wl_hi = std::max(wl_hi, out[i].v[7]);
+  }
+  plan->n_vis_planned = planned;
+  plan->n_vis_dropped = dropped;
+  plan->wl_min = wl_lo;
+  plan->n_wlayers = out.empty() ? 1 : (wl_hi - wl_lo + 1);
+
+  plan->tiles_x = (Ng + kTile - 1) / kTile;
+  plan->tiles_y = plan->tiles_x;
+
+  // batches: contiguous ranges of the sorted subgrid list (§3.4 :259-267, R18)
+  int64_t cap = par.max_batch_subgrids;
+  if (cap <= 0) {
+    const int64_t bytes_per = static_cast<int64_t>(L) * L * 4 * 8;
+    cap = std::max<int64_t>(1, (int64_t{4} << 30) / bytes_per);
+  }
+  plan->batch_capacity = std::max<int64_t>(1, std::min<int64_t>(cap, std::max<int64_t>(plan->n_subgrids, 1)));
+  plan->batches.clear();
+  for (int64_t first = 0; first < plan->n_subgrids; first += plan->batch_capacity) {
+    Batch bt;
+    bt.first = first;
+    bt.count = std::min(plan->batch_capacity, plan->n_subgrids - first);
+    build_tile_csr(plan, bt.first, bt.count, &bt.csr);
+    plan->batches.push_back(std::move(bt));
+  }
+  return IDG_OK;
+}
+
+// For subgrids [first, first+count): which adder tiles (kTile x kTile master-grid pixels of one
+// w-layer) does each overlap.  Lists are ascending in subgrid index, which fixes the summation
+// order of the adder (R18: bitwise reproducible).
+void build_tile_csr(const idg_plan* plan, int64_t first, int64_t count, TileCsr* out) {
+  const int32_t L = plan->par.subgrid_size;
+  const int32_t tx_n = plan->tiles_x, ty_n = plan->tiles_y;
+  std::vector<std::pair<int32_t, int32_t>> pairs;   // (tile id, subgrid)
+  pairs.reserve(static_cast<size_t>(count) * 4);
+  for (int64_t s = first; s < first + count; ++s) {
+    const int32_t* e = &plan->sub[static_cast<size_t>(s) * 8];
+    const int32_t x0 = e[5], y0 = e[6], layer = e[7] - plan->wl_min;
+    const int32_t tx0 = x0 / kTile, tx1 = (x0 + L - 1) / kTile;
+    const int32_t ty0 = y0 / kTile, ty1 = (y0 + L - 1) / kTile;
+    for (int32_t ty = ty0; ty <= ty1; ++ty)
+      for (int32_t tx = tx0; tx <= tx1; ++tx)
+        pairs.emplace_back((layer * ty_n + ty) * tx_n + tx, static_cast<int32_t>(s));
+  }
+  std::sort(pairs.begin(), pairs.end());
+  out->tile_ids.clear(); out->offsets.clear(); out->items.clear();
+  out->items.reserve(pairs.size());
+  for (size_t i = 0; i < pairs.size(); ++i) {
+    if (i == 0 || pairs[i].first != pairs[i - 1].first) {
+      out->tile_ids.push_back(pairs[i].first);
+      out->offsets.push_back(static_cast<int32_t>(i));
+    }
+    out->items.push_back(pairs[i].second);
+  }
+  out->offsets.push_back(static_cast<int32_t>(pairs.size()));
+}
+
+// Per-subgrid device metadata: the 8 plan fields plus stations (p, q), A-term interval and
+// grid layer index, so kernels need no second lookup.
+void fill_meta(const idg_plan* plan, std::vector<int32_t>* meta) {
+  meta->resize(static_cast<size_t>(plan->n_subgrids) * kMetaStride);
+  for (int64_t s = 0; s < plan->n_subgrids; ++s) {
+    const int32_t* e = &plan->sub[static_cast<size_t>(s) * 8];
+    int32_t* m = &(*meta)[static_cast<size_t>(s) * kMetaStride];
+    for (int i = 0; i < 8; ++i) m[i] = e[i];
+    m[8] = plan->baselines[static_cast<size_t>(e[0]) * 2 + 0];
+    m[9] = plan->baselines[static_cast<size_t>(e[0]) * 2 + 1];
+    m[10] = e[1] / plan->par.aterm_period;
+    m[11] = e[7] - plan->wl_min;
+  }
+}
+
+}  // namespace idg

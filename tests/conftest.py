@@ -24,3 +24,13 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+@pytest.fixture(scope="session")
+def idg():
+    """The Python binding with the C-ABI library built in-tree (nvcc cross-compiles on CPU boxes)."""
+    from paper_2502_17789_b200 import build
+    build.build()
+    import paper_2502_17789_b200 as pkg
+    pkg.load_library()
+    return pkg

@@ -1,0 +1,283 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element on
+the same seeded inputs.  Tolerance (BASELINE.json north_star): normalised max
+error max|gpu - oracle| / max|oracle| <= 1e-5 per subgrid (after the A-term/taper epilogue and
+after the FFT) and per subgrid's degridded visibilities; plan, adder and splitter bit-exact."""
+import numpy as np
+import pytest
+import torch
+
+import synth
+from oracle import idg_oracle as orc
+from tests.util import inner, oracle_params, random_jones
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-5
+DEV = "cuda:0"
+
+
+def nerr(gpu, ref):
+    return float(np.abs(np.asarray(gpu, np.complex128) - ref).max() / max(np.abs(ref).max(), 1e-300))
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).to(DEV)
+
+
+def setup(idg, cfg, vis="hash", aterms="config", seed=0, **plan_kw):
+    obs = synth.make_observation(cfg, vis=vis, with_aterms=(aterms == "config"))
+    if aterms == "random":
+        rng = np.random.default_rng(seed)
+        obs.aterms = random_jones(rng, (cfg.n_stations, cfg.n_intervals, cfg.subgrid_size, cfg.subgrid_size))
+    par = oracle_params(cfg)
+    plan = idg.plan_from_config(cfg, obs.uvw, obs.freqs, obs.baselines, **plan_kw)
+    sub = plan.export()
+    return obs, par, plan, sub
+
+
+CASES = [
+    ("cfg1", lambda: synth.get_config(1), "sources"),
+    ("cfg1-hash", lambda: synth.get_config(1), "hash"),
+    ("cfg2-10st", lambda: synth.scaled(synth.get_config(2), n_stations=10, n_times=16), "hash"),
+    ("cfg3-8st-layers", lambda: synth.scaled(synth.get_config(3), n_stations=8, n_times=8, n_chan=96), "hash"),
+    ("cfg4-12st", lambda: synth.scaled(synth.get_config(4), n_stations=12, n_times=8), "sources"),
+    ("L128", lambda: synth.scaled(synth.get_config(2), n_stations=6, n_times=8, n_chan=16, subgrid_size=128,
+                                  padding=24), "hash"),
+    ("ragged", lambda: synth.scaled(synth.get_config(1), n_stations=7, n_times=13, n_chan=5, aterm_period=3),
+     "hash"),
+    ("wide-rows", lambda: synth.scaled(synth.get_config(1), n_stations=5, n_times=8, n_chan=150, chan_width_hz=2e3),
+     "hash"),
+]
+IDS = [c[0] for c in CASES]
+
+
+def sample_subgrids(sub, n, seed=0):
+    """All subgrids if few, else n random ones plus the least and most occupied."""
+    if len(sub) <= n:
+        return list(range(len(sub)))
+    occ = sub[:, 2].astype(np.int64) * sub[:, 4]
+    rng = np.random.default_rng(seed)
+    pick = set(rng.choice(len(sub), n, replace=False).tolist())
+    pick.update([int(occ.argmin()), int(occ.argmax()), 0, len(sub) - 1])
+    return sorted(pick)
+
+
+@pytest.mark.parametrize("name,make,vis", CASES, ids=IDS)
+def test_gridder_and_fft_per_subgrid(idg, name, make, vis):
+    """Steps a1-a4 per subgrid, after the epilogue and after the FFT."""
+    cfg = make()
+    obs, par, plan, sub = setup(idg, cfg, vis=vis)
+    L = cfg.subgrid_size
+    n = len(sub)
+    d_vis, d_at, d_tp = dev(obs.vis), dev(obs.aterms), dev(obs.taper)
+    out_img = torch.zeros((n, 4, L, L), dtype=torch.complex64, device=DEV)
+    out_uv = torch.zeros_like(out_img)
+    idg.grid_subgrids(plan, 0, n, d_vis, d_at, d_tp, out_img, stage=idg.STAGE_GRIDDER)
+    idg.grid_subgrids(plan, 0, n, d_vis, d_at, d_tp, out_uv, stage=idg.STAGE_FFT)
+    torch.cuda.synchronize()
+    g_img = out_img.cpu().numpy()
+    g_uv = out_uv.cpu().numpy()
+    worst = (0.0, 0.0)
+    for s in sample_subgrids(sub, 12):
+        Sp, Shat = orc.grid_subgrid(par, sub[s], obs.uvw, obs.freqs, obs.vis, obs.baselines, obs.aterms, obs.taper)
+        e1 = nerr(np.moveaxis(g_img[s], 0, 2), Sp)
+        e2 = nerr(np.moveaxis(g_uv[s], 0, 2), Shat)
+        worst = (max(worst[0], e1), max(worst[1], e2))
+        assert e1 <= TOL and e2 <= TOL, (name, s, sub[s].tolist(), e1, e2)
+    print(f"{name}: worst normalised error image {worst[0]:.2e} uv {worst[1]:.2e}")
+
+
+@pytest.mark.parametrize("name,make,vis", CASES, ids=IDS)
+def test_degridder_per_subgrid(idg, name, make, vis):
+    """Steps a8-a9 per subgrid on random image-domain subgrids."""
+    cfg = make()
+    obs, par, plan, sub = setup(idg, cfg, vis=None)
+    L = cfg.subgrid_size
+    n = len(sub)
+    rng = np.random.default_rng(7)
+    picks = sample_subgrids(sub, 10)
+    S = np.zeros((n, 4, L, L), np.complex64)
+    for s in picks:
+        S[s] = (rng.standard_normal((4, L, L)) + 1j * rng.standard_normal((4, L, L))).astype(np.complex64)
+    d_S, d_at, d_tp = dev(S), dev(obs.aterms), dev(obs.taper)
+    d_vis = torch.full((cfg.n_rows, cfg.n_chan, 4), 7.0 + 0j, dtype=torch.complex64, device=DEV)
+    idg.degrid_subgrids(plan, 0, n, d_S, d_at, d_tp, d_vis)
+    torch.cuda.synchronize()
+    g = d_vis.cpu().numpy()
+    for s in picks:
+        b, t0, nt, c0, nc = (int(v) for v in sub[s][:5])
+        Mp, Mq = orc.subgrid_jones(par, sub[s], obs.baselines, obs.aterms)
+        Sp = orc.aterm_taper(np.moveaxis(S[s].astype(np.complex128), 0, 2), Mp, Mq, obs.taper)
+        ref = orc.degridder_subgrid(par, sub[s], obs.uvw, obs.freqs, Sp)
+        r0 = b * cfg.n_times + t0
+        e = nerr(g[r0:r0 + nt, c0:c0 + nc], ref)
+        assert e <= TOL, (name, s, sub[s].tolist(), e)
+
+
+@pytest.mark.parametrize("L", [32, 64, 96, 128])
+def test_subgrid_fft_matches_oracle_and_inverts(idg, L):
+    rng = np.random.default_rng(L)
+    x = (rng.standard_normal((5, L, L)) + 1j * rng.standard_normal((5, L, L))).astype(np.complex64)
+    d = dev(x)
+    idg.subgrid_fft(L, d, +1)
+    fwd = d.cpu().numpy()
+    for i in range(5):
+        ref = orc.subgrid_fft(x[i].astype(np.complex128)[:, :, None])[:, :, 0]
+        assert nerr(fwd[i], ref) < 2e-6
+    idg.subgrid_fft(L, d, -1)
+    back = d.cpu().numpy().astype(np.complex128) * (L * L)     # each direction carries 1/L^2 (R2)
+    assert nerr(back, x.astype(np.complex128)) < 2e-6
+    d2 = dev(x)
+    idg.subgrid_fft(L, d2, -1)
+    inv = d2.cpu().numpy()
+    ref = orc.subgrid_ifft(x[0].astype(np.complex128)[:, :, None])[:, :, 0]
+    assert nerr(inv[0], ref) < 2e-6
+
+
+@pytest.mark.parametrize("name,make", [(c[0], c[1]) for c in CASES[:5]], ids=IDS[:5])
+def test_adder_and_splitter_bit_exact(idg, name, make):
+    """P8: integer-valued subgrids give order-independent sums, so the tile-owner adder must
+    equal numpy's indexed add bit for bit; the splitter is a pure gather."""
+    cfg = make()
+    obs, par, plan, sub = setup(idg, cfg, vis=None, aterms="none")
+    L, Ng, n = cfg.subgrid_size, cfg.grid_size, len(sub)
+    cnt = plan.counts()
+    rng = np.random.default_rng(3)
+    S = (rng.integers(-8, 9, (n, 4, L, L)) + 1j * rng.integers(-8, 9, (n, 4, L, L))).astype(np.complex64)
+    G0 = (rng.integers(-3, 4, (cnt.n_wlayers, 4, Ng, Ng)) + 0j).astype(np.complex64)
+    d_G = dev(G0)
+    # in two ranges, to exercise first > 0
+    half = n // 2
+    idg.adder(plan, 0, half, dev(S[:half]), d_G)
+    idg.adder(plan, half, n - half, dev(S[half:]), d_G)
+    ref = G0.astype(np.complex128)
+    for s in range(n):
+        orc.adder(ref, np.moveaxis(S[s].astype(np.complex128), 0, 2), sub[s], cnt.wl_min)
+    assert np.array_equal(d_G.cpu().numpy(), ref.astype(np.complex64))
+    # splitter
+    Gr = (rng.standard_normal((cnt.n_wlayers, 4, Ng, Ng)) + 1j * rng.standard_normal((cnt.n_wlayers, 4, Ng, Ng)))
+    Gr = Gr.astype(np.complex64)
+    out = torch.zeros((n - half, 4, L, L), dtype=torch.complex64, device=DEV)
+    idg.splitter(plan, half, n - half, dev(Gr), out)
+    o = out.cpu().numpy()
+    for s in range(half, n):
+        ref_p = orc.splitter(Gr, sub[s], L, cnt.wl_min)
+        assert np.array_equal(np.moveaxis(o[s - half], 0, 2), ref_p.astype(np.complex64))
+
+
+@pytest.mark.parametrize("batch", [0, 7])
+def test_full_grid_and_degrid_config1(idg, batch):
+    """The whole path on config 1 (all 56 subgrids), single batch and ragged batches of 7."""
+    cfg = synth.get_config(1)
+    obs, par, plan, sub = setup(idg, cfg, vis="sources", max_batch_subgrids=batch)
+    cnt = plan.counts()
+    Ng = cfg.grid_size
+    d_vis, d_at, d_tp = dev(obs.vis), dev(obs.aterms), dev(obs.taper)
+    d_grid = torch.zeros((cnt.n_wlayers, 4, Ng, Ng), dtype=torch.complex64, device=DEV)
+    ws = torch.empty(plan.workspace_bytes(idg.IDG_GRID), dtype=torch.uint8, device=DEV)
+    idg.grid(plan, d_vis, d_at, d_tp, d_grid, ws)
+    torch.cuda.synchronize()
+    ref = orc.grid(par, sub, obs.uvw, obs.freqs, obs.vis, obs.baselines, obs.aterms, obs.taper)
+    assert nerr(d_grid.cpu().numpy(), ref) <= TOL
+    # bitwise reproducible (R18): atomic-free adder, fixed order
+    d_grid2 = torch.zeros_like(d_grid)
+    idg.grid(plan, d_vis, d_at, d_tp, d_grid2, ws)
+    assert torch.equal(torch.view_as_real(d_grid), torch.view_as_real(d_grid2))
+    # prediction from the oracle's grid (rounded to complex64)
+    G = ref.astype(np.complex64)
+    d_out = torch.zeros((cfg.n_rows, cfg.n_chan, 4), dtype=torch.complex64, device=DEV)
+    idg.degrid(plan, dev(G), d_at, d_tp, d_out, ws)
+    torch.cuda.synchronize()
+    vref = orc.degrid(par, sub, obs.uvw, obs.freqs, G, obs.baselines, obs.aterms, obs.taper)
+    assert nerr(d_out.cpu().numpy(), vref) <= TOL
+
+
+def test_full_path_layers_and_drops(idg):
+    """Several signed w-layers, dropped visibilities left untouched, batches not aligned to layers."""
+    cfg = synth.scaled(synth.get_config(3), n_stations=7, n_times=8, n_chan=48, grid_size=1024, cell_arcsec=120.0,
+                       w_step=4.0, ha_mid_deg=30.0)
+    obs, par, plan, sub = setup(idg, cfg, vis="hash", max_batch_subgrids=5)
+    cnt = plan.counts()
+    assert cnt.n_wlayers >= 3 and cnt.n_vis_dropped > 0 and cnt.n_subgrids > 10
+    Ng = cfg.grid_size
+    d_vis, d_at, d_tp = dev(obs.vis), dev(obs.aterms), dev(obs.taper)
+    d_grid = torch.zeros((cnt.n_wlayers, 4, Ng, Ng), dtype=torch.complex64, device=DEV)
+    ws = torch.empty(plan.workspace_bytes(), dtype=torch.uint8, device=DEV)
+    idg.grid(plan, d_vis, d_at, d_tp, d_grid, ws)
+    ref = orc.grid(par, sub, obs.uvw, obs.freqs, obs.vis, obs.baselines, obs.aterms, obs.taper)
+    assert nerr(d_grid.cpu().numpy(), ref) <= TOL
+    G = ref.astype(np.complex64)
+    sentinel = 123.0 - 5.0j
+    d_out = torch.full((cfg.n_rows, cfg.n_chan, 4), sentinel, dtype=torch.complex64, device=DEV)
+    idg.degrid(plan, dev(G), d_at, d_tp, d_out, ws)
+    vref = orc.degrid(par, sub, obs.uvw, obs.freqs, G, obs.baselines, obs.aterms, obs.taper,
+                      out=np.full((cfg.n_rows, cfg.n_chan, 4), sentinel, np.complex128))
+    got = d_out.cpu().numpy()
+    assert nerr(got, vref) <= TOL
+    covered = np.zeros((cfg.n_rows, cfg.n_chan), bool)
+    for b, t0, nt, c0, nc, *_ in sub:
+        covered[b * cfg.n_times + t0: b * cfg.n_times + t0 + nt, c0:c0 + nc] = True
+    assert np.all(got[~covered] == np.complex64(sentinel)), "dropped visibilities must stay untouched"
+
+
+def test_adjoint_on_gpu(idg):
+    """P3 on the GPU pair: <degrid(G; M), V> = <G, grid(V; M^H)> to fp32 accuracy."""
+    cfg = synth.scaled(synth.get_config(2), n_stations=8, n_times=16)
+    obs, par, plan, sub = setup(idg, cfg, vis="hash", aterms="random", seed=5)
+    cnt = plan.counts()
+    Ng = cfg.grid_size
+    rng = np.random.default_rng(11)
+    G = (rng.standard_normal((cnt.n_wlayers, 4, Ng, Ng)) + 1j * rng.standard_normal((cnt.n_wlayers, 4, Ng, Ng)))
+    G = G.astype(np.complex64)
+    MH = np.ascontiguousarray(np.conj(np.swapaxes(obs.aterms, -1, -2)))
+    ws = torch.empty(plan.workspace_bytes(), dtype=torch.uint8, device=DEV)
+    d_tp = dev(obs.taper)
+    d_pred = torch.zeros((cfg.n_rows, cfg.n_chan, 4), dtype=torch.complex64, device=DEV)
+    idg.degrid(plan, dev(G), dev(obs.aterms), d_tp, d_pred, ws)
+    d_grid = torch.zeros((cnt.n_wlayers, 4, Ng, Ng), dtype=torch.complex64, device=DEV)
+    idg.grid(plan, dev(obs.vis), dev(MH), d_tp, d_grid, ws)
+    lhs = inner(d_pred.cpu().numpy().astype(np.complex128), obs.vis.astype(np.complex128))
+    rhs = inner(G.astype(np.complex128), d_grid.cpu().numpy().astype(np.complex128))
+    rel = abs(lhs - rhs) / abs(lhs)
+    print(f"adjoint relative mismatch {rel:.2e}")
+    assert rel < 2e-5
+
+
+def test_host_buffer_calls(idg):
+    """idg_grid_host / idg_degrid_host give the device path's results through host buffers."""
+    cfg = synth.get_config(1)
+    obs, par, plan, sub = setup(idg, cfg, vis="sources", max_batch_subgrids=16)
+    cnt = plan.counts()
+    Ng = cfg.grid_size
+    arena = torch.empty(plan.host_arena_bytes(), dtype=torch.uint8, device=DEV)
+    h_vis = torch.from_numpy(obs.vis).pin_memory()
+    h_at = torch.from_numpy(obs.aterms).pin_memory()
+    h_tp = torch.from_numpy(obs.taper).pin_memory()
+    h_grid = torch.zeros((cnt.n_wlayers, 4, Ng, Ng), dtype=torch.complex64).pin_memory()
+    idg.grid_host(plan, h_vis, h_at, h_tp, h_grid, arena)
+    ref = orc.grid(par, sub, obs.uvw, obs.freqs, obs.vis, obs.baselines, obs.aterms, obs.taper)
+    assert nerr(h_grid.numpy(), ref) <= TOL
+    h_out = torch.zeros((cfg.n_rows, cfg.n_chan, 4), dtype=torch.complex64).pin_memory()
+    G = torch.from_numpy(ref.astype(np.complex64)).pin_memory()
+    idg.degrid_host(plan, G, h_at, h_tp, h_out, arena)
+    vref = orc.degrid(par, sub, obs.uvw, obs.freqs, ref.astype(np.complex64), obs.baselines, obs.aterms, obs.taper)
+    assert nerr(h_out.numpy(), vref) <= TOL
+
+
+def test_empty_and_error_paths(idg):
+    cfg = synth.get_config(1)
+    obs, par, plan, sub = setup(idg, cfg, vis="sources")
+    L = cfg.subgrid_size
+    d_vis, d_at, d_tp = dev(obs.vis), dev(obs.aterms), dev(obs.taper)
+    out = torch.zeros((1, 4, L, L), dtype=torch.complex64, device=DEV)
+    idg.grid_subgrids(plan, 3, 0, d_vis, d_at, d_tp, out)          # empty range: no-op
+    with pytest.raises(idg.IdgError, match="bad range"):
+        idg.grid_subgrids(plan, len(sub), 1, d_vis, d_at, d_tp, out)
+    small = torch.empty(16, dtype=torch.uint8, device=DEV)
+    d_grid = torch.zeros((1, 4, cfg.grid_size, cfg.grid_size), dtype=torch.complex64, device=DEV)
+    with pytest.raises(idg.IdgError, match="workspace too small"):
+        idg.grid(plan, d_vis, d_at, d_tp, d_grid, small)
+    before = idg.launch_count()
+    ws = torch.empty(plan.workspace_bytes(), dtype=torch.uint8, device=DEV)
+    idg.grid(plan, d_vis, d_at, d_tp, d_grid, ws)
+    assert idg.launch_count() == before + 3                          # gridder, fft, adder
