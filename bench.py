@@ -1,0 +1,454 @@
+"""bench.py -- the IDG hot path (grid + degrid) timed on B200, with its roofline and the oracle beside it.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one seeded synthetic observation: idg_grid
+(gridder -> A-term/taper -> subgrid FFT -> adder) followed by idg_degrid (splitter -> inverse FFT
+-> taper/A-term -> degridder) over every visibility of the workload.  `value` = visibilities that
+went through BOTH directions per second (n_vis / step time); the per-direction rates are in
+`grid_vis_per_s` / `degrid_vis_per_s`.  Workload: BASELINE.json configs[1] (MWA Phase I-like, 128
+stations, L = 64), the one the 60 % roofline target is quoted on.  Multi-GPU: the path is specified
+for one GPU (replicas only) -- with --gpus N every rank runs the same
+workload on its own GPU, no collective on the data path, value = N * n_vis / max-over-ranks time.
+
+Prints ONE JSON line on rank 0.  `--impl reference` times the fp64 numpy oracle (oracle/) on the
+host cores on a bounded sample of the same workload and prints the same line shape.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import synth  # noqa: E402
+
+METRIC = "gridded+degridded visibilities/s (grid then degrid of every visibility, 4 pols each)"
+UNIT = "vis/s"
+N_SM = 148
+FP32_LANES_PER_SM = 128          # FFMA lanes per SM per clock (micro-benchmarked)
+FP32_OPS_PER_PAIR = 18           # 16 FFMA (2x2 complex MAC) + 1 phase FFMA + 1 range-reduction FMUL
+MUFU_PER_PAIR = 2
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d["sm_max_mhz"]), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+# ---------------------------------------------------------------------------------------------
+# oracle on the host cores (cpu_baseline leg and --impl reference): a bounded sample of subgrids
+# ---------------------------------------------------------------------------------------------
+_W = {}
+
+
+def _w_grid(i):
+    from oracle import idg_oracle as orc
+    w = _W
+    _, shat = orc.grid_subgrid(w["par"], w["sub"][i], w["uvw"], w["freqs"], w["vis"], w["bl"], w["aterms"], w["taper"])
+    return i, shat
+
+
+def _w_degrid(i):
+    from oracle import idg_oracle as orc
+    w = _W
+    _, v = orc.degrid_subgrid(w["par"], w["sub"][i], w["uvw"], w["freqs"], w["grid"], w["wl_min"], w["bl"],
+                              w["aterms"], w["taper"])
+    return i, complex(v.sum())
+
+
+def oracle_params(cfg):
+    from oracle import idg_oracle as orc
+    return orc.OracleParams(grid_size=cfg.grid_size, subgrid_size=cfg.subgrid_size, padding=cfg.padding,
+                            cell_size=cfg.cell_size, w_step=cfg.w_step, n_times=cfg.n_times, n_chan=cfg.n_chan,
+                            aterm_period=cfg.aterm_period, comfort=cfg.comfort)
+
+
+def oracle_sample(cfg, obs, n_subgrids, seed):
+    """A seeded sample of the workload for the oracle: random baselines, planned by the ORACLE's own
+    planner (O1), their rows renumbered 0..n-1 so that only those baselines' uvw rows and
+    visibilities have to exist on the host.  Input marshalling only; returns a dict for
+    oracle_sample_run."""
+    from oracle import idg_oracle as orc
+    par = oracle_params(cfg)
+    rng = np.random.default_rng(seed)
+    order = rng.permutation(cfg.n_baselines)
+    per_bl = max(1, cfg.n_intervals)                      # at least one subgrid per interval
+    n_bl = int(min(cfg.n_baselines, max(1, -(-n_subgrids // per_bl))))
+    bls = np.sort(order[:n_bl])
+    rows = (bls[:, None].astype(np.int64) * cfg.n_times + np.arange(cfg.n_times)[None, :]).reshape(-1)
+    uvw = obs.uvw[rows]
+    sub, _ = orc.plan(par, uvw, obs.freqs, n_bl)          # baselines 0..n_bl-1 of the compact table
+    if len(sub) > n_subgrids:
+        keep = np.sort(rng.choice(len(sub), n_subgrids, replace=False))
+        sub = sub[keep]
+    vis = synth.source_visibilities(uvw, obs.freqs, obs.sources)
+    return dict(par=par, sub=sub, uvw=uvw, freqs=obs.freqs, vis=vis, bl=obs.baselines[bls], aterms=obs.aterms,
+                taper=obs.taper)
+
+
+def oracle_sample_run(cfg, sample, workers):
+    """Times the oracle (as it stands) over the sampled subgrids: O2-O5 then O6-O9, in a fork pool
+    of `workers` processes.  Returns (n_vis_sampled, seconds)."""
+    import multiprocessing as mp
+    from oracle import idg_oracle as orc
+    sub = sample["sub"]
+    wl_min, W = orc.layer_range(sub)
+    Ng = cfg.grid_size
+    _W.update(sample)
+    _W["wl_min"] = wl_min
+    ctx = mp.get_context("fork")
+    idx = list(range(len(sub)))
+    t0 = time.perf_counter()
+    G = np.zeros((W, 4, Ng, Ng), np.complex64)          # lazily allocated; only sampled patches are touched
+    with ctx.Pool(workers, initializer=_pool_init) as pool:
+        for i, shat in pool.imap_unordered(_w_grid, idx):
+            orc.adder(G, shat, sub[i], wl_min)
+    _W["grid"] = G
+    with ctx.Pool(workers, initializer=_pool_init) as pool:
+        chk = sum(v for _, v in pool.imap_unordered(_w_degrid, idx))
+    dt = time.perf_counter() - t0
+    _W.clear()
+    assert np.isfinite(chk.real)
+    n_vis = int((sub[:, 2].astype(np.int64) * sub[:, 4]).sum())
+    return n_vis, dt
+
+
+def host_workers():
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+
+def _pool_init():
+    try:
+        from threadpoolctl import threadpool_limits
+        _W["_limit"] = threadpool_limits(1)               # one BLAS thread per worker: the pool owns the cores
+    except Exception:
+        pass
+
+
+def calibrated_oracle(cfg, obs, target_s, seed, workers):
+    """Runs the oracle on a small probe sample, then on one sized for about `target_s` seconds of
+    wall time.  Returns (vis_per_s, n_vis, seconds, n_subgrids)."""
+    probe = oracle_sample(cfg, obs, max(2 * workers, 8), seed)
+    n_vis, dt = oracle_sample_run(cfg, probe, workers)
+    per_sub = dt / max(len(probe["sub"]), 1)
+    n = int(max(len(probe["sub"]), min(target_s / max(per_sub, 1e-6), 4096)))
+    if n > len(probe["sub"]) * 1.5:
+        sample = oracle_sample(cfg, obs, n, seed + 1)
+        n_vis, dt = oracle_sample_run(cfg, sample, workers)
+        return n_vis / dt, n_vis, dt, len(sample["sub"])
+    return n_vis / dt, n_vis, dt, len(probe["sub"])
+
+
+def workload_config(cfg):
+    return {"workload": f"BASELINE.json configs[{cfg.config_id - 1}] '{cfg.name}': {cfg.n_stations} stations, "
+                        f"{cfg.n_baselines} baselines x {cfg.n_times} times x {cfg.n_chan} chan = {cfg.n_vis} vis x 4 pol c64",
+            "subgrid_size": cfg.subgrid_size, "padding": cfg.padding, "grid_size": cfg.grid_size,
+            "aterm_period": cfg.aterm_period, "w_step": cfg.w_step,
+            "l2": "inputs larger than L2 (visibilities + subgrid stack >> 126 MB); no explicit flush"}
+
+
+def run_reference(args):
+    """--impl reference: the fp64 numpy oracle on the host cores, K steps, each a bounded seeded
+    sample of the workload (oracle/ is test infrastructure; this is its one timed use)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cfg = synth.get_config(args.config)
+    obs = synth.make_observation(cfg, vis=None)
+    workers = host_workers()
+    budget = 150.0                                         # seconds for the whole run
+    per_step = max(2.0, budget / max(args.steps + args.warmup, 1))
+    probe = oracle_sample(cfg, obs, max(2 * workers, 8), 7)
+    _, dt = oracle_sample_run(cfg, probe, workers)        # also serves as the first warm-up
+    n_sub = int(max(workers, min(per_step / max(dt / len(probe["sub"]), 1e-6), 2048)))
+    for w in range(max(args.warmup - 1, 0)):
+        oracle_sample_run(cfg, oracle_sample(cfg, obs, n_sub, 100 + w), workers)
+    tot_vis, tot_s, tot_sub = 0, 0.0, 0
+    for k in range(args.steps):
+        smp = oracle_sample(cfg, obs, n_sub, 200 + k)
+        n_vis, dt = oracle_sample_run(cfg, smp, workers)
+        tot_vis += n_vis
+        tot_s += dt
+        tot_sub += len(smp["sub"])
+    value = tot_vis / tot_s
+    sample = f"{tot_sub // max(args.steps, 1)} seeded random subgrids per step ({tot_vis // max(args.steps, 1)} vis), grid then degrid, fork pool"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_s / max(args.steps, 1),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(cfg),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": workers, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled while the timed region runs (profiling recipe)."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.FIELDS}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in self.f.read().splitlines():
+            parts = [x.strip() for x in ln.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons),
+                       samples=len(sm), power_w_max=float(max(pw)))
+        return out
+
+
+def kernel_rooflines(cfg, sub, n_wlayers, prof_ms, prof_n, steps, peaks, sm_mhz_obs):
+    """Per-kernel achieved rates over the timed region.  ALU kernels (gridder, degridder): algorithmic
+    FP32-pipe work = 18 lane-ops per (visibility, pixel) pair, counted as 2 flop each, against
+    148 SM x 128 lanes x 2 flop x max SM clock.  HBM kernels (FFT, adder, splitter): algorithmic bytes
+    against the measured copy bandwidth.  DESIGN.md "Roofline" derives every figure used here."""
+    L, Ng = cfg.subgrid_size, cfg.grid_size
+    occ = sub[:, 2].astype(np.int64) * sub[:, 4]
+    n_vis = int(occ.sum())
+    pairs = float(n_vis) * L * L
+    n_sub = len(sub)
+    flop = pairs * FP32_OPS_PER_PAIR * 2.0
+    peak_tflops = N_SM * FP32_LANES_PER_SM * 2.0 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    stack = n_sub * 4.0 * L * L * 8.0
+    grid_bytes = n_wlayers * 4.0 * Ng * Ng * 8.0
+    aterm_taper = n_sub * (2.0 * L * L * 32.0 + L * L * 4.0)
+    alg_bytes = {
+        "gridder": n_vis * 32.0 + aterm_taper + stack,
+        "degridder": n_vis * 32.0 + aterm_taper + stack,
+        "fft": 2.0 * stack, "ifft": 2.0 * stack,
+        "adder": stack + 2.0 * grid_bytes,
+        "splitter": 2.0 * stack,
+    }
+    out = {}
+    for k, ms in prof_ms.items():
+        if prof_n.get(k, 0) == 0:
+            continue
+        t = ms / 1e3 / steps                                # seconds per step in this kernel
+        e = {"ms_per_step": ms / steps, "launches_per_step": prof_n[k] / steps,
+             "hbm_gbs": alg_bytes[k] / t / 1e9, "hbm_frac": alg_bytes[k] / t / 1e9 / peaks["hbm_gbs"]}
+        if k in ("gridder", "degridder"):
+            e.update(bound="alu", tflops=flop / t / 1e12, frac=flop / t / 1e12 / peak_tflops,
+                     pairs_per_s=pairs / t,
+                     pairs_per_clk_per_sm=(pairs / t) / (N_SM * sm_mhz_obs * 1e6) if sm_mhz_obs else None,
+                     frac_at_observed_clock=(flop / t / 1e12) / (peak_tflops * sm_mhz_obs / peaks["sm_max_mhz"])
+                     if sm_mhz_obs else None)
+        else:
+            e.update(bound="hbm", frac=e["hbm_frac"])
+        out[k] = e
+    return out, peak_tflops, flop, alg_bytes
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    cfg = synth.get_config(args.config)
+    peaks = load_peaks()
+    obs = synth.make_observation(cfg, vis=None)
+
+    # the oracle beside it: rank 0, N = 1 only, BEFORE CUDA is initialised (it forks a process pool)
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        workers = host_workers()
+        v, n_vis_s, dt, n_s = calibrated_oracle(cfg, obs, args.cpu_seconds, 11, workers)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": workers, "kind": "oracle",
+                        "sample": f"{n_s} seeded random subgrids ({n_vis_s} vis) of the same workload, grid then "
+                                  f"degrid, fork pool, {dt:.1f} s wall"}
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the IDG path has no CPU fallback")
+    from paper_2502_17789_b200 import build as _build
+    _build.build()
+    import paper_2502_17789_b200 as idg
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    plan = idg.plan_from_config(cfg, obs.uvw, obs.freqs, obs.baselines)
+    sub = plan.export()
+    cnt = plan.counts()
+    Ng = cfg.grid_size
+    d_vis = synth.source_visibilities_torch(obs.uvw, obs.freqs, obs.sources, dev)
+    d_at = torch.from_numpy(obs.aterms).to(dev)
+    d_tp = torch.from_numpy(obs.taper).to(dev)
+    d_grid = torch.zeros((cnt.n_wlayers, 4, Ng, Ng), dtype=torch.complex64, device=dev)
+    d_out = torch.zeros_like(d_vis)
+    ws = torch.empty(max(plan.workspace_bytes(idg.IDG_GRID), plan.workspace_bytes(idg.IDG_DEGRID)),
+                     dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        idg.grid(plan, d_vis, d_at, d_tp, d_grid, ws, stream)
+        idg.degrid(plan, d_grid, d_at, d_tp, d_out, ws, stream)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    sampler = ClockSampler(torch.cuda.current_device()) if rank == 0 else None
+    idg.profile_read()
+    idg.profile_enable(True)
+    launches0 = idg.launch_count()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps + 1)]
+    ev[0].record(stream)
+    for k in range(args.steps):
+        idg.grid(plan, d_vis, d_at, d_tp, d_grid, ws, stream)
+        ev[2 * k + 1].record(stream)
+        idg.degrid(plan, d_grid, d_at, d_tp, d_out, ws, stream)
+        ev[2 * k + 2].record(stream)
+    barrier()
+    launches = idg.launch_count() - launches0
+    idg.profile_enable(False)
+    prof = idg.profile_read()
+    clocks = sampler.stop() if sampler else None
+    total_ms = ev[0].elapsed_time(ev[-1])
+    grid_ms = sum(ev[2 * k].elapsed_time(ev[2 * k + 1]) for k in range(args.steps)) / args.steps
+    degrid_ms = sum(ev[2 * k + 1].elapsed_time(ev[2 * k + 2]) for k in range(args.steps)) / args.steps
+    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    n_vis = cnt.n_vis_planned
+
+    # end to end through the host-buffer C-ABI calls: pinned host -> device -> pinned host, every step
+    e2e = None
+    if not args.no_e2e:
+        h_vis = d_vis.cpu().pin_memory()
+        h_at = torch.from_numpy(obs.aterms).pin_memory()
+        h_tp = torch.from_numpy(obs.taper).pin_memory()
+        h_grid = torch.zeros((cnt.n_wlayers, 4, Ng, Ng), dtype=torch.complex64).pin_memory()
+        h_out = torch.zeros((cfg.n_rows, cfg.n_chan, 4), dtype=torch.complex64).pin_memory()
+        del d_out, d_grid, ws
+        torch.cuda.empty_cache()
+        arena = torch.empty(max(plan.host_arena_bytes(idg.IDG_GRID), plan.host_arena_bytes(idg.IDG_DEGRID)),
+                            dtype=torch.uint8, device=dev)
+        n_e2e = max(1, min(args.steps, 3))
+        idg.grid_host(plan, h_vis, h_at, h_tp, h_grid, arena, stream)        # warm-up
+        idg.degrid_host(plan, h_grid, h_at, h_tp, h_out, arena, stream)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            idg.grid_host(plan, h_vis, h_at, h_tp, h_grid, arena, stream)
+            idg.degrid_host(plan, h_grid, h_at, h_tp, h_out, arena, stream)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        te = torch.tensor([dt], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        dt = float(te.item())
+        nb = lambda x: x.numel() * x.element_size()  # noqa: E731
+        h2d = (nb(h_vis) + nb(h_at) + nb(h_tp) + nb(h_grid)) * 2          # grid call + degrid call
+        d2h = nb(h_grid) + nb(h_out)
+        e2e = {"value": world * n_vis * n_e2e / dt, "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "steps": n_e2e, "ms_per_step": 1e3 * dt / n_e2e,
+               "api": "idg_grid_host + idg_degrid_host (pinned host buffers, copies inside the calls)"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+    sm_obs = clocks["sm_mhz"] if clocks else None
+    prof_ms = {k: v[0] for k, v in prof.items()}
+    prof_n = {k: v[1] for k, v in prof.items()}
+    kr, peak_tflops, flop, alg_bytes = kernel_rooflines(cfg, sub, cnt.n_wlayers, prof_ms, prof_n, args.steps, peaks,
+                                                        sm_obs)
+    dom = max(("gridder", "degridder"), key=lambda k: kr[k]["ms_per_step"])
+    roofline = {"kernel": dom, "bound": "alu", "achieved": kr[dom]["tflops"], "peak": peak_tflops,
+                "unit": "TFLOP/s", "frac": kr[dom]["frac"], "traffic": None,
+                "peak_basis": f"{N_SM} SM x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {peaks['sm_max_mhz']:.0f} MHz "
+                              f"(sm_max_mhz {peaks['source']}); work = 18 FP32-pipe ops per (vis,pixel) pair",
+                "frac_at_observed_clock": kr[dom]["frac_at_observed_clock"],
+                "hbm_frac_of_measured": kr[dom]["hbm_frac"], "hbm_peak_gbs": peaks["hbm_gbs"]}
+    line = {"metric": METRIC, "value": world * n_vis / (ms_per_step / 1e3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": workload_config(cfg), "grid_vis_per_s": n_vis / (grid_ms / 1e3),
+            "degrid_vis_per_s": n_vis / (degrid_ms / 1e3), "grid_ms": grid_ms, "degrid_ms": degrid_ms,
+            "n_subgrids": int(cnt.n_subgrids), "n_vis": int(n_vis), "roofline": roofline, "kernels": kr,
+            "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config id (1-based); default 2 = configs[1]")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="wall-time target of the cpu_baseline leg")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

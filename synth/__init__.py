@@ -21,6 +21,7 @@ from .generate import (  # noqa: F401
     make_observation,
     point_sources,
     source_visibilities,
+    source_visibilities_torch,
     station_layout,
     taper_full_1d,
     taper_subgrid,

@@ -285,3 +285,27 @@ def make_observation(cfg: Config, vis: str | None = "sources", with_aterms: bool
         raise ValueError(vis)
     A = aterms(cfg) if with_aterms else None
     return Observation(cfg, baselines(cfg.n_stations), uvw, fr, v, A, taper_subgrid(cfg), src)
+
+
+def source_visibilities_torch(uvw_rows: np.ndarray, freqs: np.ndarray, src: dict, device, chunk_rows: int = 16384):
+    """The recipe of `source_visibilities` evaluated with torch fp64 on `device`, in row chunks, for
+    the large workloads ("generate them on-device with torch in chunks").
+    Returns a torch complex64 tensor [n_rows, n_chan, 4] on `device`.  Input data only."""
+    import torch
+
+    l = torch.as_tensor(src["l"], dtype=torch.float64, device=device)
+    m = torch.as_tensor(src["m"], dtype=torch.float64, device=device)
+    n1 = -(l * l + m * m) / (1.0 + torch.sqrt(1.0 - l * l - m * m))
+    kappa = torch.as_tensor(freqs / C_LIGHT, dtype=torch.float64, device=device)
+    spec = torch.as_tensor((freqs[:, None] / src["nu0"]) ** src["alpha"][None, :], dtype=torch.float64, device=device)
+    Bf = torch.as_tensor(src["brightness"].reshape(-1, 4), dtype=torch.complex128, device=device)
+    n_rows = uvw_rows.shape[0]
+    out = torch.empty((n_rows, freqs.size, 4), dtype=torch.complex64, device=device)
+    for r0 in range(0, n_rows, chunk_rows):
+        rows = torch.as_tensor(uvw_rows[r0:r0 + chunk_rows], dtype=torch.float64, device=device)
+        geo = rows[:, 0:1] * l[None, :] + rows[:, 1:2] * m[None, :] + rows[:, 2:3] * n1[None, :]   # [rows, src]
+        for c in range(freqs.size):
+            ang = (-2.0 * math.pi) * kappa[c] * geo
+            ph = torch.complex(torch.cos(ang), torch.sin(ang)) * spec[c][None, :]
+            out[r0:r0 + chunk_rows, c, :] = (ph @ Bf).to(torch.complex64)
+    return out
