@@ -170,6 +170,17 @@ IDG_API int  idg_splitter(const idg_plan* plan, int64_t first, int64_t count, co
 IDG_API int  idg_profile_enable(int on);
 IDG_API int  idg_profile_read(double* ms_out, int64_t* launches_out);
 
+/* Empirical ALU peaks of the current device, measured the way the paper measures its Table 1
+ * (§5.1 :339-351): register-only loops timed with the SM cycle counter.  Synchronous.
+ * out_host[7], per SM per clock: [0] FFMA lane-ops, [1] FFMA2 (packed fp32x2) FMA lane-ops,
+ * [2] MUFU.EX2 lane-ops, [3] sin+cos pairs (__sincosf), [4] (visibility, pixel) pairs of the
+ * gridder's instruction mix (phase FFMA + __sincosf + 8 FFMA2 per pair), [5] the same mix with
+ * 16 scalar FFMA, [6] pairs of the operand-generation mix alone (phase FFMA + __sincosf + split of
+ * cos and sin into a tf32 head and an exact remainder: what is left on the SIMT pipes when the
+ * MACs go to the tensor cores).  These are the
+ * denominators of the ALU roofline. */
+IDG_API int  idg_measure_alu_peaks(double* out_host);
+
 /* Number of kernels the library has launched in this process (for bench.py's gpu_launches). */
 IDG_API int64_t idg_launch_count(void);
 

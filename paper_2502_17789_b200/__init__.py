@@ -24,7 +24,7 @@ SYMBOLS = (
     "idg_plan_create", "idg_plan_destroy", "idg_plan_counts", "idg_plan_export", "idg_workspace_bytes",
     "idg_grid", "idg_degrid", "idg_host_arena_bytes", "idg_grid_host", "idg_degrid_host",
     "idg_grid_subgrids", "idg_degrid_subgrids", "idg_subgrid_fft", "idg_adder", "idg_splitter",
-    "idg_profile_enable", "idg_profile_read", "idg_launch_count", "idg_last_error", "idg_version",
+    "idg_profile_enable", "idg_profile_read", "idg_measure_alu_peaks", "idg_launch_count", "idg_last_error", "idg_version",
 )
 KERNEL_KINDS = ("gridder", "fft", "adder", "splitter", "ifft", "degridder")
 
@@ -91,6 +91,8 @@ def load_library() -> ctypes.CDLL:
     lib.idg_profile_enable.restype = ctypes.c_int
     lib.idg_profile_read.argtypes = [vp, vp]
     lib.idg_profile_read.restype = ctypes.c_int
+    lib.idg_measure_alu_peaks.argtypes = [vp]
+    lib.idg_measure_alu_peaks.restype = ctypes.c_int
     lib.idg_launch_count.argtypes = []
     lib.idg_launch_count.restype = i64
     lib.idg_last_error.argtypes = []
@@ -273,6 +275,15 @@ def profile_read() -> dict:
     n = np.zeros(len(KERNEL_KINDS), np.int64)
     _check(load_library().idg_profile_read(ms.ctypes.data, n.ctypes.data), "idg_profile_read")
     return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(KERNEL_KINDS)}
+
+
+def measure_alu_peaks() -> dict:
+    """idg_measure_alu_peaks: empirical per-SM-per-clock rates of the FP32 and SFU pipes."""
+    out = np.zeros(7, np.float64)
+    _check(load_library().idg_measure_alu_peaks(out.ctypes.data), "idg_measure_alu_peaks")
+    return dict(ffma=float(out[0]), ffma2=float(out[1]), mufu_ex2=float(out[2]), sincos=float(out[3]),
+                gridder_mix_pairs=float(out[4]), gridder_mix_scalar_pairs=float(out[5]),
+                operand_gen_pairs=float(out[6]))
 
 
 def launch_count() -> int:

@@ -498,6 +498,12 @@ int idg_profile_read(double* ms_out, int64_t* launches_out) {
   return IDG_OK;
 }
 
+int idg_measure_alu_peaks(double* out_host) {
+  if (!out_host) { set_error("idg_measure_alu_peaks: null argument"); return IDG_EINVAL; }
+  IDG_CUDA(measure_alu_peaks(out_host));
+  return IDG_OK;
+}
+
 int64_t idg_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 const char* idg_last_error(void) { return g_last_error.c_str(); }

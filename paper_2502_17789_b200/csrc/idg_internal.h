@@ -12,7 +12,7 @@ namespace idg {
 
 constexpr double kSpeedOfLight = 299792458.0;
 constexpr int kMetaStride = 12;   // int32 per subgrid on the device: b,t0,nt,c0,nc,x0,y0,wl,p,q,it,layer
-constexpr int kTile = 64;         // adder tile edge in master-grid pixels
+constexpr int kTile = 32;         // adder tile edge in master-grid pixels
 
 // tile -> subgrid lists for the atomic-free adder (one CSR per batch of subgrids).
 struct TileCsr {

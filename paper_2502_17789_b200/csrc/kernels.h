@@ -44,6 +44,9 @@ cudaError_t launch_adder(const int32_t* meta, const DeviceCsr& csr, int64_t firs
 cudaError_t launch_splitter(const int32_t* meta, int64_t first, int64_t count, int L, int Ng,
                             const float2* grid, float2* subgrids, cudaStream_t stream);
 
+// Empirical FFMA / FFMA2 / MUFU rates per SM clock (peaks.cu); synchronous.
+cudaError_t measure_alu_peaks(double* out5);
+
 void count_launch(int n = 1);
 
 }  // namespace idg

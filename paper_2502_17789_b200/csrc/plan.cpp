@@ -167,16 +167,24 @@ void build_tile_csr(const idg_plan* plan, int64_t first, int64_t count, TileCsr*
         pairs.emplace_back((layer * ty_n + ty) * tx_n + tx, static_cast<int32_t>(s));
   }
   std::sort(pairs.begin(), pairs.end());
+  // group by tile (subgrids ascending within a tile), then emit the tiles heaviest first so the
+  // longest lists start early (the order of TILES does not affect any sum)
+  struct Run { int32_t tile; size_t beg, end; };
+  std::vector<Run> runs;
+  for (size_t i = 0; i < pairs.size(); ++i) {
+    if (i == 0 || pairs[i].first != pairs[i - 1].first) runs.push_back({pairs[i].first, i, i});
+    runs.back().end = i + 1;
+  }
+  std::stable_sort(runs.begin(), runs.end(),
+                   [](const Run& a, const Run& b) { return (a.end - a.beg) > (b.end - b.beg); });
   out->tile_ids.clear(); out->offsets.clear(); out->items.clear();
   out->items.reserve(pairs.size());
-  for (size_t i = 0; i < pairs.size(); ++i) {
-    if (i == 0 || pairs[i].first != pairs[i - 1].first) {
-      out->tile_ids.push_back(pairs[i].first);
-      out->offsets.push_back(static_cast<int32_t>(i));
-    }
-    out->items.push_back(pairs[i].second);
+  for (const Run& r : runs) {
+    out->tile_ids.push_back(r.tile);
+    out->offsets.push_back(static_cast<int32_t>(out->items.size()));
+    for (size_t i = r.beg; i < r.end; ++i) out->items.push_back(pairs[i].second);
   }
-  out->offsets.push_back(static_cast<int32_t>(pairs.size()));
+  out->offsets.push_back(static_cast<int32_t>(out->items.size()));
 }
 
 // Per-subgrid device metadata: the 8 plan fields plus stations (p, q), A-term interval and
