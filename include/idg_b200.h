@@ -170,6 +170,15 @@ IDG_API int  idg_splitter(const idg_plan* plan, int64_t first, int64_t count, co
 IDG_API int  idg_profile_enable(int on);
 IDG_API int  idg_profile_read(double* ms_out, int64_t* launches_out);
 
+/* Kernel variant of the two direct-sum kernels (process-wide; kind = IDG_K_GRIDDER or
+ * IDG_K_DEGRIDDER).  IDG_VARIANT_SIMT: all arithmetic on the FP32/SFU pipes (packed FFMA2).
+ * IDG_VARIANT_TENSOR: the phasor matrix is generated on the SIMT pipes and the 2x2 complex MACs run
+ * on the tensor cores (tcgen05, split-tf32 operands, fp32 accumulation).  Both meet the 1e-5 bar. */
+#define IDG_VARIANT_SIMT   0
+#define IDG_VARIANT_TENSOR 1
+IDG_API int  idg_set_kernel_variant(int kind, int variant);
+IDG_API int  idg_get_kernel_variant(int kind);
+
 /* Empirical ALU peaks of the current device, measured the way the paper measures its Table 1
  * (§5.1 :339-351): register-only loops timed with the SM cycle counter.  Synchronous.
  * out_host[7], per SM per clock: [0] FFMA lane-ops, [1] FFMA2 (packed fp32x2) FMA lane-ops,

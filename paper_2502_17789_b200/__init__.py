@@ -14,7 +14,8 @@ from dataclasses import dataclass
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libidg_b200.so")
+# IDG_B200_LIBRARY overrides the in-tree library (used to compare differently compiled builds)
+LIB_PATH = os.environ.get("IDG_B200_LIBRARY") or os.path.join(_HERE, "libidg_b200.so")
 
 IDG_GRID, IDG_DEGRID = 0, 1
 STAGE_GRIDDER, STAGE_FFT = 0, 1
@@ -24,7 +25,8 @@ SYMBOLS = (
     "idg_plan_create", "idg_plan_destroy", "idg_plan_counts", "idg_plan_export", "idg_workspace_bytes",
     "idg_grid", "idg_degrid", "idg_host_arena_bytes", "idg_grid_host", "idg_degrid_host",
     "idg_grid_subgrids", "idg_degrid_subgrids", "idg_subgrid_fft", "idg_adder", "idg_splitter",
-    "idg_profile_enable", "idg_profile_read", "idg_measure_alu_peaks", "idg_launch_count", "idg_last_error", "idg_version",
+    "idg_profile_enable", "idg_profile_read", "idg_set_kernel_variant", "idg_get_kernel_variant",
+    "idg_measure_alu_peaks", "idg_launch_count", "idg_last_error", "idg_version",
 )
 KERNEL_KINDS = ("gridder", "fft", "adder", "splitter", "ifft", "degridder")
 
@@ -91,6 +93,10 @@ def load_library() -> ctypes.CDLL:
     lib.idg_profile_enable.restype = ctypes.c_int
     lib.idg_profile_read.argtypes = [vp, vp]
     lib.idg_profile_read.restype = ctypes.c_int
+    lib.idg_set_kernel_variant.argtypes = [ctypes.c_int, ctypes.c_int]
+    lib.idg_set_kernel_variant.restype = ctypes.c_int
+    lib.idg_get_kernel_variant.argtypes = [ctypes.c_int]
+    lib.idg_get_kernel_variant.restype = ctypes.c_int
     lib.idg_measure_alu_peaks.argtypes = [vp]
     lib.idg_measure_alu_peaks.restype = ctypes.c_int
     lib.idg_launch_count.argtypes = []
@@ -275,6 +281,18 @@ def profile_read() -> dict:
     n = np.zeros(len(KERNEL_KINDS), np.int64)
     _check(load_library().idg_profile_read(ms.ctypes.data, n.ctypes.data), "idg_profile_read")
     return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(KERNEL_KINDS)}
+
+
+VARIANT_SIMT, VARIANT_TENSOR = 0, 1
+
+
+def set_kernel_variant(kind: str, variant: int) -> None:
+    """idg_set_kernel_variant: kind in ("gridder", "degridder"); variant VARIANT_SIMT | VARIANT_TENSOR."""
+    _check(load_library().idg_set_kernel_variant(KERNEL_KINDS.index(kind), int(variant)), "idg_set_kernel_variant")
+
+
+def get_kernel_variant(kind: str) -> int:
+    return int(load_library().idg_get_kernel_variant(KERNEL_KINDS.index(kind)))
 
 
 def measure_alu_peaks() -> dict:

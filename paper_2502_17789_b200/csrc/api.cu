@@ -14,6 +14,7 @@ namespace idg {
 
 static thread_local std::string g_last_error;
 static std::atomic<int64_t> g_launches{0};
+static std::atomic<int> g_variant[IDG_K_COUNT] = {};
 
 void set_error(const std::string& msg) { g_last_error = msg; }
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
@@ -141,8 +142,14 @@ SubgridJob make_job(const idg_plan* plan, const DeviceState* d, int64_t first, i
   j.first = first; j.count = count;
   j.subgrid_size = plan->par.subgrid_size; j.grid_size = plan->par.grid_size;
   j.n_times = plan->par.n_times; j.n_chan = plan->par.n_chan; j.n_intervals = plan->n_intervals;
+  j.max_nt = plan->par.n_times < plan->par.aterm_period ? plan->par.n_times : plan->par.aterm_period;
   j.image_size = plan->image_size; j.w_step = plan->par.w_step;
   return j;
+}
+
+cudaError_t run_gridder(const SubgridJob& job, const float4* vis, float2* out, cudaStream_t stream) {
+  return g_variant[IDG_K_GRIDDER].load() == IDG_VARIANT_TENSOR ? launch_gridder_tc(job, vis, out, stream)
+                                                                : launch_gridder(job, vis, out, stream);
 }
 
 bool range_ok(const idg_plan* plan, int64_t first, int64_t count) {
@@ -268,7 +275,7 @@ int idg_grid(const idg_plan* plan, const void* vis_dev, const void* aterms_dev, 
     const Batch& bt = plan->batches[i];
     const SubgridJob job = make_job(plan, d, bt.first, bt.count, aterms_dev, taper_dev);
     { ProfScope ps(IDG_K_GRIDDER, stream);
-      IDG_CUDA(launch_gridder(job, static_cast<const float4*>(vis_dev), stack, stream)); }
+      IDG_CUDA(run_gridder(job, static_cast<const float4*>(vis_dev), stack, stream)); }
     { ProfScope ps(IDG_K_FFT, stream);
       IDG_CUDA(launch_subgrid_fft(L, bt.count * 4, stack, +1, stream)); }
     { ProfScope ps(IDG_K_ADDER, stream);
@@ -400,7 +407,7 @@ int idg_grid_subgrids(const idg_plan* plan, int64_t first, int64_t count, const 
   if (rc != IDG_OK) return rc;
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   const SubgridJob job = make_job(plan, d, first, count, aterms_dev, taper_dev);
-  IDG_CUDA(launch_gridder(job, static_cast<const float4*>(vis_dev), static_cast<float2*>(subgrids_dev), stream));
+  IDG_CUDA(run_gridder(job, static_cast<const float4*>(vis_dev), static_cast<float2*>(subgrids_dev), stream));
   if (stage == IDG_STAGE_FFT)
     IDG_CUDA(launch_subgrid_fft(plan->par.subgrid_size, count * 4, static_cast<float2*>(subgrids_dev), +1, stream));
   return IDG_OK;
@@ -496,6 +503,21 @@ int idg_profile_read(double* ms_out, int64_t* launches_out) {
   }
   if (first_err != cudaSuccess) return cuda_fail(first_err, "idg_profile_read");
   return IDG_OK;
+}
+
+int idg_set_kernel_variant(int kind, int variant) {
+  if ((kind != IDG_K_GRIDDER && kind != IDG_K_DEGRIDDER) ||
+      (variant != IDG_VARIANT_SIMT && variant != IDG_VARIANT_TENSOR)) {
+    set_error("idg_set_kernel_variant: bad kind or variant");
+    return IDG_EINVAL;
+  }
+  g_variant[kind].store(variant);
+  return IDG_OK;
+}
+
+int idg_get_kernel_variant(int kind) {
+  if (kind < 0 || kind >= IDG_K_COUNT) return IDG_EINVAL;
+  return g_variant[kind].load();
 }
 
 int idg_measure_alu_peaks(double* out_host) {

@@ -20,6 +20,7 @@ struct SubgridJob {
   int64_t first;            // first subgrid (global index)
   int64_t count;
   int32_t subgrid_size, grid_size, n_times, n_chan, n_intervals;
+  int32_t max_nt;           // upper bound of nt over subgrids = min(n_times, aterm_period)
   double image_size;        // S
   double w_step;
 };
@@ -27,6 +28,9 @@ struct SubgridJob {
 // steps a1-a3: stage visibilities, direct sum (Eq. 10), A-term sandwich and taper.
 // out [count, 4, L, L] complex64.
 cudaError_t launch_gridder(const SubgridJob& job, const float4* vis, float2* out, cudaStream_t stream);
+
+// the same with the 2x2 complex MACs on the tensor cores (tcgen05, A operand generated into TMEM)
+cudaError_t launch_gridder_tc(const SubgridJob& job, const float4* vis, float2* out, cudaStream_t stream);
 
 // steps a8-a9: taper + A-term on image-domain subgrids, then the per-visibility sum (Eq. 13).
 // in [count, 4, L, L] complex64; vis [n_rows, n_chan, 4] complex64.
