@@ -44,6 +44,9 @@ namespace {
 #ifndef IDG_TC_DG
 #define IDG_TC_DG 4
 #endif
+#ifndef IDG_TC_NA
+#define IDG_TC_NA 3
+#endif
 
 constexpr int kTileM = 128;           // pixels per MMA tile = compute threads
 constexpr int kThreadsTc = kTileM + 32;
@@ -62,22 +65,23 @@ __device__ __forceinline__ float tf32_round(float x) {
   return __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
 }
 
-// G = tiles per CTA, KC = visibilities per chunk (8 or 16), DG = chunks per accumulator group
-template <int L, int G, int KC, int DG>
+// G = tiles per CTA, KC = visibilities per chunk (8 or 16), DG = chunks per accumulator group,
+// NA = depth of the (A in TMEM, B in shared memory) operand ring
+template <int L, int G, int KC, int DG, int NA>
 __global__ void __launch_bounds__(kThreadsTc) gridder_tc_kernel(const SubgridJob job, const float4* __restrict__ vis,
                                                                 float2* __restrict__ out) {
-  static_assert((L * L) % (kTileM * G) == 0 && (KC == 8 || KC == 16), "shape");
+  static_assert((L * L) % (kTileM * G) == 0 && (KC == 8 || KC == 16) && NA >= 3 && NA <= 4, "shape");
   constexpr int PIECES = (L * L) / (kTileM * G);
   constexpr int A_COLS = 4 * KC;                       // per buffer: heads [0, 2KC), remainders [2KC, 4KC)
-  constexpr int D_COL = 2 * A_COLS;                    // two accumulators of 16 columns
-  constexpr int TMEM_COLS = (D_COL + 32) <= 128 ? 128 : 256;
+  constexpr int D_COL = NA * A_COLS;                   // two accumulators of 16 columns
+  constexpr int TMEM_COLS = (D_COL + 32) <= 128 ? 128 : ((D_COL + 32) <= 256 ? 256 : 512);
   constexpr int B_BYTES = KC * 128;                    // 2 KC k-rows x 16 columns x 4 bytes
   constexpr uint32_t IDESC = tc::make_idesc_tf32(kTileM, 16);
 
-  __shared__ __align__(1024) unsigned char sB[2][B_BYTES];
+  __shared__ __align__(1024) unsigned char sB[NA][B_BYTES];
   __shared__ __align__(16) float sdk[kMaxChanTc];
   __shared__ RowDataTc srow[kMaxRowsTc];
-  __shared__ __align__(8) uint64_t bars[8];            // full[2], empty[2], dfull[2], dempty[2]
+  __shared__ __align__(8) uint64_t bars[2 * NA + 4];   // full[NA], empty[NA], dfull[2], dempty[2]
   __shared__ uint32_t s_tmem;
 
   const int tid = threadIdx.x, warp = tid / 32, lane = tid % 32;
@@ -88,13 +92,15 @@ __global__ void __launch_bounds__(kThreadsTc) gridder_tc_kernel(const SubgridJob
   const int sp = m[8], sq = m[9], it = m[10];
   const int64_t row0 = static_cast<int64_t>(b) * job.n_times + t0;
 
-  const uint32_t bar_full = tc::smem_u32(&bars[0]), bar_empty = tc::smem_u32(&bars[2]);
-  const uint32_t bar_dfull = tc::smem_u32(&bars[4]), bar_dempty = tc::smem_u32(&bars[6]);
+  const uint32_t bar_full = tc::smem_u32(&bars[0]), bar_empty = tc::smem_u32(&bars[NA]);
+  const uint32_t bar_dfull = tc::smem_u32(&bars[2 * NA]), bar_dempty = tc::smem_u32(&bars[2 * NA + 2]);
 
   if (tid == 0) {
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < NA; ++i) {
       tc::mbar_init(bar_full + 8 * i, kTileM);
       tc::mbar_init(bar_empty + 8 * i, 1);
+    }
+    for (int i = 0; i < 2; ++i) {
       tc::mbar_init(bar_dfull + 8 * i, 1);
       tc::mbar_init(bar_dempty + 8 * i, kTileM);
     }
@@ -133,28 +139,37 @@ __global__ void __launch_bounds__(kThreadsTc) gridder_tc_kernel(const SubgridJob
   tc::fence_after_thread_sync();
   const uint32_t tmem = s_tmem;
 
+  const int cpr = (nc + KC - 1) / KC;                  // chunks per table row
+  const int nchunks = nt * cpr;                        // chunks per tile
+  const int total = nchunks * G;                       // the CTA's chunk sequence g = 0 .. total-1
+
   if (warp == 4) {
     // ===== service warp: stage B, issue MMAs =====
     // lane -> items (visibility j, polarisation p) of a chunk; element (n, k) of the N x K operand
     // lives at ((k/4)*2 + n/8)*128 + (n%8)*16 + (k%4)*4 bytes; rows (2j, 2j+1) of one column are adjacent
     constexpr int ITEMS = KC * 4 / 32;
-    float2 pre[ITEMS];
-    auto b_load = [&](int r, int cc) {
+    constexpr int PD = 4;                              // visibility prefetch distance in chunks
+    float2 ring[PD][ITEMS];
+    int pr = 0, pcc = 0, pn = 0;                       // next chunk to prefetch: row, first channel, index
+    auto prefetch = [&](float2 (&dst)[ITEMS]) {
 #pragma unroll
       for (int i = 0; i < ITEMS; ++i) {
         const int item = lane + 32 * i, j = item >> 2, p = item & 3;
-        pre[i] = make_float2(0.f, 0.f);
-        if (cc + j < nc)
-          pre[i] = __ldg(reinterpret_cast<const float2*>(vis) + ((row0 + r) * job.n_chan + c0 + cc + j) * 4 + p);
+        dst[i] = make_float2(0.f, 0.f);
+        if (pn < total && pcc + j < nc)
+          dst[i] = __ldg(reinterpret_cast<const float2*>(vis) + ((row0 + pr) * job.n_chan + c0 + pcc + j) * 4 + p);
       }
+      ++pn;
+      pcc += KC;
+      if (pcc >= nc) { pcc = 0; if (++pr == nt) pr = 0; }
     };
-    auto b_store = [&](int buf) {
-      float* Bf = reinterpret_cast<float*>(&sB[buf][0]);
+    auto b_store = [&](const float2 (&src)[ITEMS], int slot) {
+      float* Bf = reinterpret_cast<float*>(&sB[slot][0]);
 #pragma unroll
       for (int i = 0; i < ITEMS; ++i) {
         const int item = lane + 32 * i, j = item >> 2, p = item & 3;
-        const float hr = tf32_round(pre[i].x), hi = tf32_round(pre[i].y);
-        const float lr = tf32_round(pre[i].x - hr), li = tf32_round(pre[i].y - hi);
+        const float hr = tf32_round(src[i].x), hi = tf32_round(src[i].y);
+        const float lr = tf32_round(src[i].x - hr), li = tf32_round(src[i].y - hi);
         auto at2 = [&](int n) -> float2* {
           return reinterpret_cast<float2*>(&Bf[((j >> 1) * 2 + (n >> 3)) * 32 + (n & 7) * 4 + (j & 1) * 2]);
         };
@@ -165,51 +180,64 @@ __global__ void __launch_bounds__(kThreadsTc) gridder_tc_kernel(const SubgridJob
       }
       tc::fence_proxy_async();
     };
+    auto shift_ring = [&]() {
+#pragma unroll
+      for (int d = 0; d + 1 < PD; ++d)
+#pragma unroll
+        for (int i = 0; i < ITEMS; ++i) ring[d][i] = ring[d + 1][i];
+    };
 
-    b_load(0, 0);
-    b_store(0);
+    // ring[d] holds the visibilities of chunk (staged + d).  B is staged S = NA - 2 chunks ahead of the
+    // MMAs, so the slot being overwritten was read two chunks ago and the wait below rarely blocks.
+    constexpr int S = NA - 2;
+#pragma unroll
+    for (int d = 0; d < PD; ++d) prefetch(ring[d]);
+    int staged = 0, sslot = 0, sphase = 0;             // next chunk to stage, its slot and ring phase
+#pragma unroll
+    for (int d = 0; d < S; ++d) {
+      if (staged < total) b_store(ring[0], sslot);
+      shift_ring();
+      prefetch(ring[PD - 1]);
+      ++staged;
+      if (++sslot == NA) { sslot = 0; sphase ^= 1; }
+    }
     __syncwarp();
-    int g = 0, q = 0;
-    for (int tile = 0; tile < G; ++tile) {
-      int cig = 0;
-      for (int r = 0; r < nt; ++r) {
-        for (int cc = 0; cc < nc; cc += KC) {
-          const int buf = g & 1;
-          // next chunk in the CTA's sequence (wraps to the next tile)
-          int nr = r, ncc = cc + KC;
-          if (ncc >= nc) { ncc = 0; if (++nr == nt) nr = 0; }
-          const bool tile_last = (r == nt - 1) && (cc + KC >= nc);
-          const bool has_next = !(tile_last && tile == G - 1);
-          if (has_next) b_load(nr, ncc);
-          if (lane == 0) {
-            if (cig == 0 && q >= 2) {                  // accumulator q & 1 drained (group q - 2)
-              tc::mbar_wait(bar_dempty + 8 * (q & 1), ((q - 2) >> 1) & 1);
-              tc::fence_after_thread_sync();
-            }
-            tc::mbar_wait(bar_full + 8 * buf, (g >> 1) & 1);
-            tc::fence_after_thread_sync();
-            const uint32_t a0 = tmem + buf * A_COLS;
-            const uint32_t d0 = tmem + D_COL + 16 * (q & 1);
-            const uint32_t bbase = tc::smem_u32(&sB[buf][0]);
-#pragma unroll
-            for (int part = 0; part < 2; ++part)
-#pragma unroll
-              for (int ks = 0; ks < KC / 4; ++ks) {
-                const uint64_t bdesc = tc::make_smem_desc(bbase + ks * 512, 256, 128);
-                tc::mma_tf32_ts(d0, a0 + part * 2 * KC + ks * 8, bdesc, IDESC, (cig > 0 || part > 0 || ks > 0) ? 1u : 0u);
-              }
-            tc::mma_commit(bar_empty + 8 * buf);
-            if (cig == DG - 1 || tile_last) tc::mma_commit(bar_dfull + 8 * (q & 1));
-            // B[buf ^ 1] was read by the MMAs of chunk g - 1
-            if (has_next && g >= 1) tc::mbar_wait(bar_empty + 8 * (buf ^ 1), ((g - 1) >> 1) & 1);
-          }
-          __syncwarp();
-          if (has_next) b_store(buf ^ 1);
-          __syncwarp();
-          ++g;
-          if (++cig == DG || tile_last) { cig = 0; ++q; }
+
+    int slot = 0, phase = 0, ci = 0, cig = 0, q = 0;
+    for (int g = 0; g < total; ++g) {
+      const bool tile_last = ci == nchunks - 1;
+      if (lane == 0) {
+        if (cig == 0 && q >= 2) {                      // accumulator q & 1 drained (group q - 2)
+          tc::mbar_wait(bar_dempty + 8 * (q & 1), ((q - 2) >> 1) & 1);
+          tc::fence_after_thread_sync();
         }
+        tc::mbar_wait(bar_full + 8 * slot, phase);
+        tc::fence_after_thread_sync();
+        const uint32_t a0 = tmem + slot * A_COLS;
+        const uint32_t d0 = tmem + D_COL + 16 * (q & 1);
+        const uint32_t bbase = tc::smem_u32(&sB[slot][0]);
+#pragma unroll
+        for (int part = 0; part < 2; ++part)
+#pragma unroll
+          for (int ks = 0; ks < KC / 4; ++ks) {
+            const uint64_t bdesc = tc::make_smem_desc(bbase + ks * 512, 256, 128);
+            tc::mma_tf32_ts(d0, a0 + part * 2 * KC + ks * 8, bdesc, IDESC, (cig > 0 || part > 0 || ks > 0) ? 1u : 0u);
+          }
+        tc::mma_commit(bar_empty + 8 * slot);
+        if (cig == DG - 1 || tile_last) tc::mma_commit(bar_dfull + 8 * (q & 1));
+        // the slot of chunk `staged` = g + S was last read by the MMAs of chunk staged - NA
+        if (staged < total && staged >= NA) tc::mbar_wait(bar_empty + 8 * sslot, sphase ^ 1);
       }
+      __syncwarp();
+      if (staged < total) b_store(ring[0], sslot);
+      shift_ring();
+      prefetch(ring[PD - 1]);
+      ++staged;
+      if (++sslot == NA) { sslot = 0; sphase ^= 1; }
+      __syncwarp();
+      if (++slot == NA) { slot = 0; phase ^= 1; }
+      if (++ci == nchunks) ci = 0;
+      if (++cig == DG || tile_last) { cig = 0; ++q; }
     }
   } else {
     // ===== compute threads: one pixel of the current tile each =====
@@ -232,7 +260,7 @@ __global__ void __launch_bounds__(kThreadsTc) gridder_tc_kernel(const SubgridJob
       for (int n = 0; n < 8; ++n) acc[n] += __uint_as_float(d[n]) + __uint_as_float(d[n + 8]);
     };
 
-    int g = 0, q = 0;
+    int g = 0, q = 0, slot = 0, phase = 0;             // chunk index, group index, ring slot and ring phase
     for (int tile = 0; tile < G; ++tile) {
       const int pix = (piece * G + tile) * kTileM + tid;
       const int ix = pix % L - L / 2, iy = pix / L - L / 2;
@@ -247,9 +275,8 @@ __global__ void __launch_bounds__(kThreadsTc) gridder_tc_kernel(const SubgridJob
         const int32_t bf = rd.alpha_fix * ix + rd.beta_fix * iy;                    // wraps: exact mod 1 cycle
         const float pb = fmaf(rd.gamma, np, static_cast<float>(bf) * 1.4629180792671596e-9f);   // 2 pi / 2^32
         for (int cc = 0; cc < nc; cc += KC) {
-          const int buf = g & 1;
-          if (g >= 2) tc::mbar_wait(bar_empty + 8 * buf, ((g - 2) >> 1) & 1);       // A[buf] read by chunk g - 2
-          const uint32_t abuf = tmem + lane_base + buf * A_COLS;
+          if (g >= NA) tc::mbar_wait(bar_empty + 8 * slot, phase ^ 1);              // A[slot] read by chunk g - NA
+          const uint32_t abuf = tmem + lane_base + slot * A_COLS;
 #pragma unroll
           for (int half = 0; half < KC / 8; ++half) {
             uint32_t hi[16], lo[16];
@@ -271,8 +298,9 @@ __global__ void __launch_bounds__(kThreadsTc) gridder_tc_kernel(const SubgridJob
           }
           tc::tmem_wait_st();
           tc::fence_before_thread_sync();
-          tc::mbar_arrive(bar_full + 8 * buf);
+          tc::mbar_arrive(bar_full + 8 * slot);
           ++g;
+          if (++slot == NA) { slot = 0; phase ^= 1; }
           const bool tile_last = (r == nt - 1) && (cc + KC >= nc);
           if (++cig == DG || tile_last) {
             if (gin > 0) drain(q - 1);                 // the previous group: its MMAs finished long ago
@@ -306,12 +334,12 @@ constexpr int tiles_per_cta(int L, int want) {
   return g;
 }
 
-template <int L, int G, int KC, int DG>
+template <int L, int G, int KC, int DG, int NA>
 cudaError_t launch(const SubgridJob& job, const float4* vis, float2* out, cudaStream_t stream) {
   constexpr int PIECES = (L * L) / (kTileM * G);
   const int64_t blocks = job.count * PIECES;
   if (blocks == 0) return cudaSuccess;
-  gridder_tc_kernel<L, G, KC, DG><<<static_cast<unsigned>(blocks), kThreadsTc, 0, stream>>>(job, vis, out);
+  gridder_tc_kernel<L, G, KC, DG, NA><<<static_cast<unsigned>(blocks), kThreadsTc, 0, stream>>>(job, vis, out);
   count_launch();
   return cudaGetLastError();
 }
@@ -322,10 +350,10 @@ cudaError_t launch_gridder_tc(const SubgridJob& job, const float4* vis, float2* 
   // shapes whose per-subgrid constants do not fit the kernel's shared-memory tables take the SIMT kernel
   if (job.n_chan > kMaxChanTc - 16 || job.max_nt > kMaxRowsTc) return launch_gridder(job, vis, out, stream);
   switch (job.subgrid_size) {
-    case 32:  return launch<32, tiles_per_cta(32, IDG_TC_G), IDG_TC_KC, IDG_TC_DG>(job, vis, out, stream);
-    case 64:  return launch<64, tiles_per_cta(64, IDG_TC_G), IDG_TC_KC, IDG_TC_DG>(job, vis, out, stream);
-    case 96:  return launch<96, tiles_per_cta(96, IDG_TC_G), IDG_TC_KC, IDG_TC_DG>(job, vis, out, stream);
-    case 128: return launch<128, tiles_per_cta(128, IDG_TC_G), IDG_TC_KC, IDG_TC_DG>(job, vis, out, stream);
+    case 32:  return launch<32, tiles_per_cta(32, IDG_TC_G), IDG_TC_KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
+    case 64:  return launch<64, tiles_per_cta(64, IDG_TC_G), IDG_TC_KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
+    case 96:  return launch<96, tiles_per_cta(96, IDG_TC_G), IDG_TC_KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
+    case 128: return launch<128, tiles_per_cta(128, IDG_TC_G), IDG_TC_KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
     default:  return cudaErrorInvalidValue;
   }
 }
