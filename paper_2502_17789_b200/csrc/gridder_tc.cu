@@ -51,7 +51,7 @@ namespace {
 #define IDG_TC_NG 4
 #endif
 #ifndef IDG_TC_DG
-#define IDG_TC_DG 4
+#define IDG_TC_DG 6
 #endif
 #ifndef IDG_TC_NA
 #define IDG_TC_NA 3
@@ -90,6 +90,8 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, 1)
   constexpr int TMEM_COLS = NG * GCOLS <= 128 ? 128 : (NG * GCOLS <= 256 ? 256 : 512);
   static_assert(NG * GCOLS <= 512, "TMEM");
   constexpr int CHUNK_BYTES = KC * 128;                // 2 KC k-rows x 16 columns x 4 bytes
+  static_assert(DG % NA == 0, "an accumulator group is a whole number of ring revolutions");
+  constexpr int RPG = DG / NA;                         // revolutions per accumulator group
   constexpr int NBAR = 2 * NA + 4;                     // per group: full[NA], empty[NA], dfull[2], dempty[2]
   constexpr uint32_t IDESC = tc::make_idesc_tf32(kTileM, 16);
 
@@ -173,10 +175,8 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, 1)
   // dempty[p] at + 16 NA + 16.  `opaque` keeps them in registers.
   const uint32_t gbar = tc::opaque(bar0 + 8 * mygroup * NBAR);
   const uint32_t gtmem = tc::opaque(tmem + mygroup * GCOLS + (static_cast<uint32_t>((warp & 3) * 32) << 16));
-  int g = 0, q = 0, slot = 0;
-  uint32_t phase = 0;
-  int sq_ = 0, sslot = 0;                              // the service warps' own copies (warp-uniform)
-  uint32_t sphase = 0;
+  int q = 0, revs = 0;                                 // accumulator groups closed, ring revolutions done
+  uint32_t phase = 0;                                  // parity of the current revolution
 
   const int tpix = tid & (kTileM - 1);
   const float4* __restrict__ ap = job.aterms + (static_cast<int64_t>(sp) * job.n_intervals + it) * (L * L * 2);
@@ -192,9 +192,12 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, 1)
     // --- step a1: the B operand of the segment's visibilities.  Element (n, k) of a chunk's N x K
     // operand lives at ((k/4)*2 + n/8)*128 + (n%8)*16 + (k%4)*4 bytes; k = 2 j + {cos, sin}.
     if (seg > 0) __syncthreads();                      // every MMA of the previous segment was drained
-    for (int idx = tid; idx < nchunks * KC * 4; idx += NTHREADS) {
-      const int p = idx & 3, j = (idx >> 2) % KC, ci = idx / (KC * 4);
-      const int r = r_begin + ci / cpr, cc = (ci % cpr) * KC;
+    // One warp per 8 visibilities x 4 polarisations, so the row / channel split is once per warp.
+    constexpr int UPC = KC / 8;
+    for (int u = warp; u < nchunks * UPC; u += NTHREADS / 32) {
+      const int ci = u / UPC, j = (u % UPC) * 8 + ((tid & 31) >> 2), p = tid & 3;
+      const int rr = ci / cpr;
+      const int r = r_begin + rr, cc = (ci - rr * cpr) * KC;
       float2 v = make_float2(0.f, 0.f);
       if (cc + j < nc) v = __ldg(reinterpret_cast<const float2*>(vis) + ((row0 + r) * job.n_chan + c0 + cc + j) * 4 + p);
       const float hr = tf32_round(v.x), hi = tf32_round(v.y);
@@ -211,44 +214,54 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, 1)
     tc::fence_proxy_async();
     __syncthreads();
 
+    // The chunk stream of a tile is walked in ring revolutions of NA slots (slot = position in the
+    // unrolled body); an accumulator group is RPG revolutions.  Slots past the tile's last chunk still
+    // cycle their barriers, without stores or MMAs.
+    const int nrev = (nchunks + NA - 1) / NA;
     if (gi >= NG) {
-      // ===== service warp of group `mygroup`: warp-uniform control flow, lane 0 issues =====
+      // ===== service warp of group `mygroup`: warp-uniform control flow, one elected lane issues =====
       // every operand below derives from warp-shuffled values, so it stays in uniform registers
       const uint32_t bbase = __shfl_sync(0xffffffffu, tc::smem_u32(sB), 0);
       const uint32_t gt = __shfl_sync(0xffffffffu, tmem, 0) + mygroup * GCOLS;
       const uint32_t sbar = __shfl_sync(0xffffffffu, bar0, 0) + 8 * mygroup * NBAR;
       const int n_u = __shfl_sync(0xffffffffu, nchunks, 0);
+      const int nrev_u = (n_u + NA - 1) / NA;
       for (int round = 0; round < ROUNDS; ++round) {
-        int cig = 0;
-        for (int ci = 0; ci < n_u; ++ci) {
-          const bool group_last = cig == DG - 1 || ci == n_u - 1;
-          if (cig == 0 && sq_ >= 2)                    // accumulator sq_ & 1 drained (group sq_ - 2)
-            tc::mbar_wait(sbar + 16 * NA + 16 + 8 * (sq_ & 1), ((sq_ - 2) >> 1) & 1);
-          tc::mbar_wait(sbar + 8 * sslot, sphase);
-          tc::fence_after_thread_sync();
-          const uint32_t a0 = gt + sslot * A_COLS;
-          const uint32_t d0 = gt + D_COL + 16 * (sq_ & 1);
-          const uint64_t bdesc0 = tc::make_smem_desc(bbase + ci * CHUNK_BYTES, 256, 128);
-          if (tc::elect_one()) {
+        int rig = 0;
+        for (int rev = 0; rev < nrev_u; ++rev) {
+          const bool group_last = rig == RPG - 1 || rev == nrev_u - 1;
+          const uint32_t d0 = gt + D_COL + 16 * (q & 1);
+          if (rig == 0 && q >= 2)                      // accumulator q & 1 drained (group q - 2)
+            tc::mbar_wait(sbar + 16 * NA + 16 + 8 * (q & 1), ((q - 2) >> 1) & 1);
 #pragma unroll
-            for (int part = 0; part < 2; ++part)
+          for (int s = 0; s < NA; ++s) {
+            const int ci = rev * NA + s;
+            tc::mbar_wait(sbar + 8 * s, phase);
+            tc::fence_after_thread_sync();
+            const uint64_t bdesc0 = tc::make_smem_desc(bbase + ci * CHUNK_BYTES, 256, 128);
+            if (tc::elect_one()) {
+              if (ci < n_u) {
 #pragma unroll
-              for (int ks = 0; ks < KC / 4; ++ks)
-                tc::mma_tf32_ts(d0, a0 + part * 2 * KC + ks * 8, bdesc0 + ks * (512 >> 4), IDESC,
-                                (cig > 0 || part > 0 || ks > 0) ? 1u : 0u);
-            tc::mma_commit(sbar + 8 * NA + 8 * sslot);
-            if (group_last) tc::mma_commit(sbar + 16 * NA + 8 * (sq_ & 1));
+                for (int part = 0; part < 2; ++part)
+#pragma unroll
+                  for (int ks = 0; ks < KC / 4; ++ks)
+                    tc::mma_tf32_ts(d0, gt + s * A_COLS + part * 2 * KC + ks * 8, bdesc0 + ks * (512 >> 4), IDESC,
+                                    (rig > 0 || s > 0 || part > 0 || ks > 0) ? 1u : 0u);
+              }
+              tc::mma_commit(sbar + 8 * NA + 8 * s);
+              if (s == NA - 1 && group_last) tc::mma_commit(sbar + 16 * NA + 8 * (q & 1));
+            }
+            __syncwarp();
           }
-          __syncwarp();
-          if (++sslot == NA) { sslot = 0; sphase ^= 1; }
-          if (group_last) { cig = 0; ++sq_; } else { ++cig; }
+          phase ^= 1;
+          if (group_last) { rig = 0; ++q; } else { ++rig; }
         }
       }
     } else {
       // ===== compute threads: one pixel of the group's current tile each =====
       float acc[8], pacc[8];
       int ppix = -1;                                   // tile whose last accumulator group is still in flight
-      uint32_t hand = 0;                               // full barrier of the slot stored but not yet handed over
+      bool pending = false;                            // the ring's last slot is stored but not yet handed over
 
       auto drain = [&](int qq, float (&dst)[8]) {
         tc::mbar_wait(gbar + 16 * NA + 8 * (qq & 1), (qq >> 1) & 1);
@@ -285,71 +298,88 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, 1)
           for (int p = 0; p < 4; ++p) o[p * L * L + pix] = x[p];
         }
       };
-      auto hand_off = [&]() {
+      auto hand_off = [&](uint32_t full_bar) {
         tc::tmem_wait_st();
         tc::fence_before_thread_sync();
-        tc::mbar_arrive(hand);
+        tc::mbar_arrive(full_bar);
       };
 
-      uint32_t cur_bar = gbar + 8 * slot, cur_a = gtmem + slot * A_COLS;
       for (int round = 0; round < ROUNDS; ++round) {
         const int pix = (round * NG + gi) * kTileM + tpix;
         const int ix = pix % L - L / 2, iy = pix / L - L / 2;
         const float np = job.nprime[pix];
 #pragma unroll
         for (int n = 0; n < 8; ++n) acc[n] = 0.f;
-        int cig = 0, gin = 0;                          // chunks in the current group, groups closed in this tile
-        int left = nchunks;                            // chunks of this tile still to store
-        for (int r = r_begin; r < r_end; ++r) {
-          // per-(row, pixel) slope and offset of the phase; amortised over the row's channels
+        // per-(row, pixel) slope and offset of the phase; amortised over the row's channels
+        float pa, pb;
+        auto row_setup = [&](int r) {
           const RowDataTc rd = srow[r];
-          const float pa = fmaf(rd.vs, static_cast<float>(iy), fmaf(rd.ws, np, rd.us * static_cast<float>(ix)));
+          pa = fmaf(rd.vs, static_cast<float>(iy), fmaf(rd.ws, np, rd.us * static_cast<float>(ix)));
           const int32_t bf = rd.alpha_fix * ix + rd.beta_fix * iy;                  // wraps: exact mod 1 cycle
-          const float pb = fmaf(rd.gamma, np, static_cast<float>(bf) * 1.4629180792671596e-9f);   // 2 pi / 2^32
-          uint32_t dk_addr = sdk_addr;
-          for (int cc = 0; cc < nc; cc += KC) {
+          pb = fmaf(rd.gamma, np, static_cast<float>(bf) * 1.4629180792671596e-9f);   // 2 pi / 2^32
+        };
+        int r = r_begin, cc = 0;
+        row_setup(r);
+        uint32_t dk_addr = sdk_addr;
+        int rig = 0, gin = 0;                          // revolutions in the current group, groups closed in this tile
+        int left = nchunks;                            // chunks of this tile still to store
+        for (int rev = 0; rev < nrev; ++rev) {
+          const bool need_wait = revs > 0;             // slots were used before: wait for their MMAs
+#pragma unroll
+          for (int s = 0; s < NA; ++s) {
+            const bool valid = left > 0;
             uint32_t hi[KC / 8][16], lo[KC / 8][16];
+            if (valid) {
 #pragma unroll
-            for (int half = 0; half < KC / 8; ++half) {
-              const float4 dka = tc::lds128(dk_addr + half * 32);
-              const float4 dkb = tc::lds128(dk_addr + half * 32 + 16);
-              const float dk[8] = {dka.x, dka.y, dka.z, dka.w, dkb.x, dkb.y, dkb.z, dkb.w};
+              for (int half = 0; half < KC / 8; ++half) {
+                const float4 dka = tc::lds128(dk_addr + half * 32);
+                const float4 dkb = tc::lds128(dk_addr + half * 32 + 16);
+                const float dk[8] = {dka.x, dka.y, dka.z, dka.w, dkb.x, dkb.y, dkb.z, dkb.w};
 #pragma unroll
-              for (int j = 0; j < 8; ++j) {
-                float s, c;
-                __sincosf(fmaf(pa, dk[j], pb), &s, &c);
-                const float ch = tf32_head(c), sh = tf32_head(s);
-                hi[half][2 * j] = __float_as_uint(ch);
-                hi[half][2 * j + 1] = __float_as_uint(sh);
-                lo[half][2 * j] = __float_as_uint(c - ch);
-                lo[half][2 * j + 1] = __float_as_uint(s - sh);
+                for (int j = 0; j < 8; ++j) {
+                  float sn, cs;
+                  __sincosf(fmaf(pa, dk[j], pb), &sn, &cs);
+                  const float ch = tf32_head(cs), sh = tf32_head(sn);
+                  hi[half][2 * j] = __float_as_uint(ch);
+                  hi[half][2 * j + 1] = __float_as_uint(sh);
+                  lo[half][2 * j] = __float_as_uint(cs - ch);
+                  lo[half][2 * j + 1] = __float_as_uint(sn - sh);
+                }
               }
             }
-            dk_addr += KC * 4;
-            if (hand != 0) hand_off();                 // the previous chunk: its stores finished long ago
-            if (g >= NA) tc::mbar_wait(cur_bar + 8 * NA, phase ^ 1);                // slot read by chunk g - NA
+            // the previous slot: its stores finished long ago
+            if (s > 0) hand_off(gbar + 8 * (s - 1));
+            else if (pending) hand_off(gbar + 8 * (NA - 1));
+            if (need_wait) tc::mbar_wait(gbar + 8 * NA + 8 * s, phase ^ 1);          // MMAs of the last revolution
+            if (valid) {
 #pragma unroll
-            for (int half = 0; half < KC / 8; ++half) {
-              tc::tmem_st16(cur_a + half * 16, hi[half]);
-              tc::tmem_st16(cur_a + 2 * KC + half * 16, lo[half]);
-            }
-            hand = cur_bar;
-            ++g;
-            cur_bar += 8;
-            cur_a += A_COLS;
-            if (++slot == NA) { slot = 0; phase ^= 1; cur_bar = gbar; cur_a = gtmem; }
-            --left;
-            if (++cig == DG || left == 0) {
-              // group q closes; group q - 1 was handed over DG chunks ago, so its MMAs are done
-              if (ppix >= 0) {
-                drain(q - 1, pacc);
-                finalize(pacc, ppix);
-                ppix = -1;
-              } else if (gin > 0) {
-                drain(q - 1, acc);
+              for (int half = 0; half < KC / 8; ++half) {
+                tc::tmem_st16(gtmem + s * A_COLS + half * 16, hi[half]);
+                tc::tmem_st16(gtmem + s * A_COLS + 2 * KC + half * 16, lo[half]);
               }
-              cig = 0; ++q; ++gin;
+              --left;
+              dk_addr += KC * 4;
+              cc += KC;
+              if (cc >= nc) {
+                cc = 0;
+                dk_addr = sdk_addr;
+                if (++r < r_end) row_setup(r);
+              }
             }
+          }
+          pending = true;
+          phase ^= 1;
+          ++revs;
+          if (++rig == RPG || rev == nrev - 1) {
+            // group q closes; group q - 1 was handed over a group ago, so its MMAs are done
+            if (ppix >= 0) {
+              drain(q - 1, pacc);
+              finalize(pacc, ppix);
+              ppix = -1;
+            } else if (gin > 0) {
+              drain(q - 1, acc);
+            }
+            rig = 0; ++q; ++gin;
           }
         }
         // the tile's last group is drained inside the next tile
@@ -357,7 +387,8 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, 1)
         for (int n = 0; n < 8; ++n) pacc[n] = acc[n];
         ppix = pix;
       }
-      hand_off();
+      hand_off(gbar + 8 * (NA - 1));
+      pending = false;
       drain(q - 1, pacc);
       finalize(pacc, ppix);
     }
