@@ -173,9 +173,12 @@ IDG_API int  idg_profile_read(double* ms_out, int64_t* launches_out);
 /* Kernel variant of the two direct-sum kernels (process-wide; kind = IDG_K_GRIDDER or
  * IDG_K_DEGRIDDER).  IDG_VARIANT_SIMT: all arithmetic on the FP32/SFU pipes (packed FFMA2).
  * IDG_VARIANT_TENSOR: the phasor matrix is generated on the SIMT pipes and the 2x2 complex MACs run
- * on the tensor cores (tcgen05, split-tf32 operands, fp32 accumulation).  Both meet the 1e-5 bar. */
+ * on the tensor cores (tcgen05, split-tf32 operands, fp32 accumulation).  Both meet the 1e-5 bar.
+ * IDG_VARIANT_AUTO (the default): per launch, the tensor-core kernel when at least 80 % of its
+ * 8-channel chunks carry visibilities (and the shape fits its shared-memory tables), else SIMT. */
 #define IDG_VARIANT_SIMT   0
 #define IDG_VARIANT_TENSOR 1
+#define IDG_VARIANT_AUTO   2
 IDG_API int  idg_set_kernel_variant(int kind, int variant);
 IDG_API int  idg_get_kernel_variant(int kind);
 

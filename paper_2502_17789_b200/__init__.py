@@ -283,11 +283,11 @@ def profile_read() -> dict:
     return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(KERNEL_KINDS)}
 
 
-VARIANT_SIMT, VARIANT_TENSOR = 0, 1
+VARIANT_SIMT, VARIANT_TENSOR, VARIANT_AUTO = 0, 1, 2
 
 
 def set_kernel_variant(kind: str, variant: int) -> None:
-    """idg_set_kernel_variant: kind in ("gridder", "degridder"); variant VARIANT_SIMT | VARIANT_TENSOR."""
+    """idg_set_kernel_variant: kind in ("gridder", "degridder"); variant VARIANT_SIMT | VARIANT_TENSOR | VARIANT_AUTO."""
     _check(load_library().idg_set_kernel_variant(KERNEL_KINDS.index(kind), int(variant)), "idg_set_kernel_variant")
 
 

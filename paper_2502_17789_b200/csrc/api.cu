@@ -14,7 +14,7 @@ namespace idg {
 
 static thread_local std::string g_last_error;
 static std::atomic<int64_t> g_launches{0};
-static std::atomic<int> g_variant[IDG_K_COUNT] = {};
+static std::atomic<int> g_variant[IDG_K_COUNT] = {IDG_VARIANT_AUTO, 0, 0, 0, 0, IDG_VARIANT_AUTO};
 
 void set_error(const std::string& msg) { g_last_error = msg; }
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
@@ -147,9 +147,26 @@ SubgridJob make_job(const idg_plan* plan, const DeviceState* d, int64_t first, i
   return j;
 }
 
-cudaError_t run_gridder(const SubgridJob& job, const float4* vis, float2* out, cudaStream_t stream) {
-  return g_variant[IDG_K_GRIDDER].load() == IDG_VARIANT_TENSOR ? launch_gridder_tc(job, vis, out, stream)
-                                                                : launch_gridder(job, vis, out, stream);
+// Fraction of the tensor-core gridder's 8-channel chunks that carry visibilities, over a subgrid range:
+// rows of few channels leave most of a chunk empty, and the SIMT kernel, which has no padding, wins.
+double tensor_fill(const idg_plan* plan, int64_t first, int64_t count) {
+  double used = 0.0, padded = 0.0;
+  for (int64_t s = first; s < first + count; ++s) {
+    const int32_t* m = &plan->sub[s * 8];
+    used += static_cast<double>(m[2]) * m[4];
+    padded += static_cast<double>(m[2]) * ((m[4] + 7) / 8 * 8);
+  }
+  return padded > 0.0 ? used / padded : 0.0;
+}
+
+constexpr double kTensorFillMin = 0.8;
+
+cudaError_t run_gridder(const idg_plan* plan, const SubgridJob& job, const float4* vis, float2* out,
+                        cudaStream_t stream) {
+  int v = g_variant[IDG_K_GRIDDER].load();
+  if (v == IDG_VARIANT_AUTO)
+    v = tensor_fill(plan, job.first, job.count) >= kTensorFillMin ? IDG_VARIANT_TENSOR : IDG_VARIANT_SIMT;
+  return v == IDG_VARIANT_TENSOR ? launch_gridder_tc(job, vis, out, stream) : launch_gridder(job, vis, out, stream);
 }
 
 bool range_ok(const idg_plan* plan, int64_t first, int64_t count) {
@@ -275,7 +292,7 @@ int idg_grid(const idg_plan* plan, const void* vis_dev, const void* aterms_dev, 
     const Batch& bt = plan->batches[i];
     const SubgridJob job = make_job(plan, d, bt.first, bt.count, aterms_dev, taper_dev);
     { ProfScope ps(IDG_K_GRIDDER, stream);
-      IDG_CUDA(run_gridder(job, static_cast<const float4*>(vis_dev), stack, stream)); }
+      IDG_CUDA(run_gridder(plan, job, static_cast<const float4*>(vis_dev), stack, stream)); }
     { ProfScope ps(IDG_K_FFT, stream);
       IDG_CUDA(launch_subgrid_fft(L, bt.count * 4, stack, +1, stream)); }
     { ProfScope ps(IDG_K_ADDER, stream);
@@ -407,7 +424,7 @@ int idg_grid_subgrids(const idg_plan* plan, int64_t first, int64_t count, const 
   if (rc != IDG_OK) return rc;
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   const SubgridJob job = make_job(plan, d, first, count, aterms_dev, taper_dev);
-  IDG_CUDA(run_gridder(job, static_cast<const float4*>(vis_dev), static_cast<float2*>(subgrids_dev), stream));
+  IDG_CUDA(run_gridder(plan, job, static_cast<const float4*>(vis_dev), static_cast<float2*>(subgrids_dev), stream));
   if (stage == IDG_STAGE_FFT)
     IDG_CUDA(launch_subgrid_fft(plan->par.subgrid_size, count * 4, static_cast<float2*>(subgrids_dev), +1, stream));
   return IDG_OK;
@@ -507,7 +524,7 @@ int idg_profile_read(double* ms_out, int64_t* launches_out) {
 
 int idg_set_kernel_variant(int kind, int variant) {
   if ((kind != IDG_K_GRIDDER && kind != IDG_K_DEGRIDDER) ||
-      (variant != IDG_VARIANT_SIMT && variant != IDG_VARIANT_TENSOR)) {
+      (variant != IDG_VARIANT_SIMT && variant != IDG_VARIANT_TENSOR && variant != IDG_VARIANT_AUTO)) {
     set_error("idg_set_kernel_variant: bad kind or variant");
     return IDG_EINVAL;
   }

@@ -47,8 +47,16 @@ CASES = [
      "hash"),
     ("wide-rows", lambda: synth.scaled(synth.get_config(1), n_stations=5, n_times=8, n_chan=150, chan_width_hz=2e3),
      "hash"),
+    # more visibilities per subgrid than the tensor-core gridder keeps in shared memory: segmented path
+    ("long-rows", lambda: synth.scaled(synth.get_config(1), n_stations=4, n_times=8, n_chan=220, chan_width_hz=1e3),
+     "hash"),
 ]
 IDS = [c[0] for c in CASES]
+
+
+def request_variant(idg, variant):
+    """Select the gridder kernel for one test; conftest restores the default afterwards."""
+    idg.set_kernel_variant("gridder", {"simt": idg.VARIANT_SIMT, "tensor": idg.VARIANT_TENSOR}[variant])
 
 
 def sample_subgrids(sub, n, seed=0):
@@ -62,9 +70,11 @@ def sample_subgrids(sub, n, seed=0):
     return sorted(pick)
 
 
+@pytest.mark.parametrize("variant", ["simt", "tensor"])
 @pytest.mark.parametrize("name,make,vis", CASES, ids=IDS)
-def test_gridder_and_fft_per_subgrid(idg, name, make, vis):
-    """Steps a1-a4 per subgrid, after the epilogue and after the FFT."""
+def test_gridder_and_fft_per_subgrid(idg, name, make, vis, variant):
+    """Steps a1-a4 per subgrid, after the epilogue and after the FFT, for both gridder kernels."""
+    request_variant(idg, variant)
     cfg = make()
     obs, par, plan, sub = setup(idg, cfg, vis=vis)
     L = cfg.subgrid_size
