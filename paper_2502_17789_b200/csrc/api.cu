@@ -159,7 +159,27 @@ double tensor_fill(const idg_plan* plan, int64_t first, int64_t count) {
   return padded > 0.0 ? used / padded : 0.0;
 }
 
+// The same for the tensor-core degridder, whose MMA rows are tiles of 128 visibilities.
+double tensor_fill_degrid(const idg_plan* plan, int64_t first, int64_t count) {
+  double used = 0.0, padded = 0.0;
+  for (int64_t s = first; s < first + count; ++s) {
+    const int32_t* m = &plan->sub[s * 8];
+    const int64_t k = static_cast<int64_t>(m[2]) * m[4];
+    used += static_cast<double>(k);
+    padded += static_cast<double>((k + 127) / 128 * 128);
+  }
+  return padded > 0.0 ? used / padded : 0.0;
+}
+
 constexpr double kTensorFillMin = 0.8;
+
+cudaError_t run_degridder(const idg_plan* plan, const SubgridJob& job, const float2* in, float4* vis,
+                          cudaStream_t stream) {
+  int v = g_variant[IDG_K_DEGRIDDER].load();
+  if (v == IDG_VARIANT_AUTO)
+    v = tensor_fill_degrid(plan, job.first, job.count) >= kTensorFillMin ? IDG_VARIANT_TENSOR : IDG_VARIANT_SIMT;
+  return v == IDG_VARIANT_TENSOR ? launch_degridder_tc(job, in, vis, stream) : launch_degridder(job, in, vis, stream);
+}
 
 cudaError_t run_gridder(const idg_plan* plan, const SubgridJob& job, const float4* vis, float2* out,
                         cudaStream_t stream) {
@@ -324,7 +344,7 @@ int idg_degrid(const idg_plan* plan, const void* grid_dev, const void* aterms_de
     { ProfScope ps(IDG_K_IFFT, stream);
       IDG_CUDA(launch_subgrid_fft(L, bt.count * 4, stack, -1, stream)); }
     { ProfScope ps(IDG_K_DEGRIDDER, stream);
-      IDG_CUDA(launch_degridder(job, stack, static_cast<float4*>(vis_dev), stream)); }
+      IDG_CUDA(run_degridder(plan, job, stack, static_cast<float4*>(vis_dev), stream)); }
   }
   return IDG_OK;
 }
@@ -439,7 +459,7 @@ int idg_degrid_subgrids(const idg_plan* plan, int64_t first, int64_t count, cons
   int rc = ensure_device(plan, &d);
   if (rc != IDG_OK) return rc;
   const SubgridJob job = make_job(plan, d, first, count, aterms_dev, taper_dev);
-  IDG_CUDA(launch_degridder(job, static_cast<const float2*>(subgrids_dev), static_cast<float4*>(vis_dev),
+  IDG_CUDA(run_degridder(plan, job, static_cast<const float2*>(subgrids_dev), static_cast<float4*>(vis_dev),
                             static_cast<cudaStream_t>(cuda_stream)));
   return IDG_OK;
 }

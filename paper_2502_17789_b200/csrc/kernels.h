@@ -36,6 +36,9 @@ cudaError_t launch_gridder_tc(const SubgridJob& job, const float4* vis, float2* 
 // in [count, 4, L, L] complex64; vis [n_rows, n_chan, 4] complex64.
 cudaError_t launch_degridder(const SubgridJob& job, const float2* in, float4* vis, cudaStream_t stream);
 
+// the same with the MACs on the tensor cores (thread = visibility, pixels streamed through shared memory)
+cudaError_t launch_degridder_tc(const SubgridJob& job, const float2* in, float4* vis, cudaStream_t stream);
+
 // steps a4 / a7: centred L x L DFT of n_planes planes in place, scaled by 1/L^2.
 cudaError_t launch_subgrid_fft(int L, int64_t n_planes, float2* planes, int direction, cudaStream_t stream);
 

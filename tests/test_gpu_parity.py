@@ -54,9 +54,9 @@ CASES = [
 IDS = [c[0] for c in CASES]
 
 
-def request_variant(idg, variant):
-    """Select the gridder kernel for one test; conftest restores the default afterwards."""
-    idg.set_kernel_variant("gridder", {"simt": idg.VARIANT_SIMT, "tensor": idg.VARIANT_TENSOR}[variant])
+def request_variant(idg, variant, kind="gridder"):
+    """Select the kernel of one direct-sum step for one test; conftest restores the default afterwards."""
+    idg.set_kernel_variant(kind, {"simt": idg.VARIANT_SIMT, "tensor": idg.VARIANT_TENSOR}[variant])
 
 
 def sample_subgrids(sub, n, seed=0):
@@ -97,9 +97,11 @@ def test_gridder_and_fft_per_subgrid(idg, name, make, vis, variant):
     print(f"{name}: worst normalised error image {worst[0]:.2e} uv {worst[1]:.2e}")
 
 
+@pytest.mark.parametrize("variant", ["simt", "tensor"])
 @pytest.mark.parametrize("name,make,vis", CASES, ids=IDS)
-def test_degridder_per_subgrid(idg, name, make, vis):
-    """Steps a8-a9 per subgrid on random image-domain subgrids."""
+def test_degridder_per_subgrid(idg, name, make, vis, variant):
+    """Steps a8-a9 per subgrid on random image-domain subgrids, for both degridder kernels."""
+    request_variant(idg, variant, kind="degridder")
     cfg = make()
     obs, par, plan, sub = setup(idg, cfg, vis=None)
     L = cfg.subgrid_size
