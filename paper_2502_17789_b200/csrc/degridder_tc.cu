@@ -11,8 +11,8 @@
 // live in registers) and the pixels are the contraction.  Operands are split into tf32 heads and
 // fp32 remainders and the accumulators are drained every DG chunks exactly as in the gridder.
 //
-// One CTA per subgrid: NG groups of 128 compute threads, one service warp per group, one producer warp.
-//   producer warp    streams the subgrid through shared memory in stages of 256 pixels: loads the four
+// One CTA per subgrid: NG groups of 128 compute threads, one service warp per group, two producer warps.
+//   producer warps   stream the subgrid through shared memory in stages of 256 pixels: loads the four
 //                    polarisation planes, applies taper and A-terms once per pixel and writes the B
 //                    operand (heads and remainders, canonical K-major core matrices) plus n'(pixel).
 //   compute group    owns a tile of 128 visibilities (thread = visibility = MMA row = TMEM lane) and a
@@ -51,8 +51,13 @@ constexpr int kTileV = 128;           // visibilities per MMA tile = threads per
 constexpr int kKC = 8;                // pixels per chunk
 constexpr int kStagePix = 256;        // pixels per shared-memory stage
 constexpr int kStageChunks = kStagePix / kKC;
-constexpr int kChunkBytes = kKC * 128;
-constexpr int kStageBBytes = kStageChunks * kChunkBytes;   // 32 KB
+// B operand layout: canonical K-major core matrices (8 n-rows x 16 B), the two n-groups of a k-group 128 B
+// apart, k-groups (2 pixels x {cos, sin}) kKgBytes apart: 16 B of padding per k-group spread the
+// producer's stores over all banks (without it every lane of a store hits the same two).
+constexpr int kKgBytes = 272;
+constexpr int kChunkBytes = (kKC / 2) * kKgBytes;          // 1088
+constexpr int kStageBBytes = kStageChunks * kChunkBytes;   // 34 KB
+constexpr int kProducers = 2;                              // producer warps, each half of every stage
 
 __device__ __forceinline__ float dtc_head(float x) { return __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
 __device__ __forceinline__ float dtc_round(float x) {
@@ -60,7 +65,7 @@ __device__ __forceinline__ float dtc_round(float x) {
 }
 
 template <int L, int NG, int DG, int NA, int NS>
-__global__ void __launch_bounds__(NG* kTileV + NG * 32 + 32, 1)
+__global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, 1)
     degridder_tc_kernel(const SubgridJob job, const float2* __restrict__ in, float4* __restrict__ vis) {
   static_assert((L * L) % kStagePix == 0 && L % kKC == 0 && NG == 4 && (NS & (NS - 1)) == 0, "shape");
   static_assert(DG % NA == 0, "an accumulator group is a whole number of ring revolutions");
@@ -106,7 +111,7 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + 32, 1)
       }
     }
     for (int i = 0; i < NS; ++i) {
-      tc::mbar_init(bar_sfull + 8 * i, 1);
+      tc::mbar_init(bar_sfull + 8 * i, kProducers);
       tc::mbar_init(bar_sempty + 8 * i, NG);
     }
     tc::fence_barrier_init();
@@ -143,13 +148,17 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + 32, 1)
       const float4* __restrict__ ap = job.aterms + (static_cast<int64_t>(sp) * job.n_intervals + it) * (L * L * 2);
       const float4* __restrict__ aq = job.aterms + (static_cast<int64_t>(sq) * job.n_intervals + it) * (L * L * 2);
       const float2* __restrict__ sub = in + sg * 4 * L * L;
+      const int pw = uwarp - NG * 5;                   // producer warp index
       for (int st = 0; st < NSTAGES; ++st) {
         const int gst = sc0 + st, slot = gst & (NS - 1);
         if (gst >= NS) tc::mbar_wait(bar_sempty + 8 * slot, ((gst / NS) - 1) & 1);
         float* Bs = reinterpret_cast<float*>(sB + slot * kStageBBytes);
+#ifdef IDG_DTC_FAKE_PRODUCER
+        if (gst < NS)
+#endif
 #pragma unroll 2
-        for (int i = 0; i < kStagePix / 32; ++i) {
-          const int lp = i * 32 + lane, pix = st * kStagePix + lp;
+        for (int i = 0; i < kStagePix / (32 * kProducers); ++i) {
+          const int lp = (pw * (kStagePix / (32 * kProducers)) + i) * 32 + lane, pix = st * kStagePix + lp;
           float2 x[4], z[4];
 #pragma unroll
           for (int p = 0; p < 4; ++p) x[p] = __ldg(&sub[p * L * L + pix]);
@@ -157,12 +166,12 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + 32, 1)
           sandwich(x, __ldg(&ap[pix * 2]), __ldg(&ap[pix * 2 + 1]), __ldg(&aq[pix * 2]), __ldg(&aq[pix * 2 + 1]),
                    __ldg(&job.taper[pix]), z);
           snp[slot * kStagePix + lp] = __ldg(&job.nprime[pix]);
-          // element (n, k) of a chunk's N x K operand lives at ((k/4)*2 + n/8)*128 + (n%8)*16 + (k%4)*4
+          // element (n, k) of a chunk's N x K operand lives at (k/4)*kKgBytes + (n/8)*128 + (n%8)*16 + (k%4)*4
           // bytes; k = 2 j + {cos, sin}, j = pixel within the chunk
           const int ci = lp >> 3, j = lp & 7;
           float* Bf = Bs + ci * (kChunkBytes / 4);
           auto at2 = [&](int n) -> float2* {
-            return reinterpret_cast<float2*>(&Bf[((j >> 1) * 2 + (n >> 3)) * 32 + (n & 7) * 4 + (j & 1) * 2]);
+            return reinterpret_cast<float2*>(&Bf[(j >> 1) * (kKgBytes / 4) + (n >> 3) * 32 + (n & 7) * 4 + (j & 1) * 2]);
           };
 #pragma unroll
           for (int p = 0; p < 4; ++p) {
@@ -209,14 +218,14 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + 32, 1)
             tc::mbar_wait(sbar + 8 * s, phase);
             tc::fence_after_thread_sync();
             const uint64_t bdesc0 =
-                tc::make_smem_desc(bbase + slot * kStageBBytes + ((part << lgn) + cl) * kChunkBytes, 256, 128);
+                tc::make_smem_desc(bbase + slot * kStageBBytes + ((part << lgn) + cl) * kChunkBytes, kKgBytes, 128);
             if (tc::elect_one()) {
               if (valid) {
 #pragma unroll
                 for (int pt = 0; pt < 2; ++pt)
 #pragma unroll
                   for (int ks = 0; ks < kKC / 4; ++ks)
-                    tc::mma_tf32_ts(d0, gt + s * A_COLS + pt * 2 * kKC + ks * 8, bdesc0 + ks * (512 >> 4), IDESC,
+                    tc::mma_tf32_ts(d0, gt + s * A_COLS + pt * 2 * kKC + ks * 8, bdesc0 + ks * ((2 * kKgBytes) >> 4), IDESC,
                                     (rig > 0 || s > 0 || pt > 0 || ks > 0) ? 1u : 0u);
               }
               tc::mma_commit(sbar + 8 * NA + 8 * s);
@@ -275,6 +284,9 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + 32, 1)
       const uint32_t snp_addr = tc::smem_u32(snp);
       uint32_t np_addr = 0;                            // n' of the next chunk's pixels
       float fx0 = 0.f, fy = 0.f;                       // pixel offsets of the next chunk's first pixel
+      // cl = chunks left in my share of the current stage; kept in plain registers (`opaque`)
+      const int ncs_r = static_cast<int>(tc::opaque(static_cast<uint32_t>(ncs)));
+      const int lp0 = static_cast<int>(tc::opaque(static_cast<uint32_t>((part << lgn) * kKC)));
       int left = total, cl = 0, st = 0, rig = 0, gin = 0;
       for (int rev = 0; rev < nrev; ++rev) {
         const bool need_wait = revs > 0;               // slots were used before: wait for their MMAs
@@ -287,23 +299,38 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + 32, 1)
               // a new stage: wait for the producer, find my share of its pixels
               const int gst = sc0 + st, slot = gst & (NS - 1);
               tc::mbar_wait(bar_sfull + 8 * slot, (gst / NS) & 1);
-              const int lp0 = (part << lgn) * kKC, pix0 = st * kStagePix + lp0;
+              const int pix0 = st * kStagePix + lp0;
               np_addr = snp_addr + (slot * kStagePix + lp0) * 4;
               fx0 = static_cast<float>(pix0 % L - L / 2);
               fy = static_cast<float>(pix0 / L - L / 2);
+              ++st;
+              cl = ncs_r;
             }
             const float4 na = tc::lds128(np_addr), nb = tc::lds128(np_addr + 16);
-            const float npv[8] = {na.x, na.y, na.z, na.w, nb.x, nb.y, nb.z, nb.w};
+            const float2 np2[4] = {make_float2(na.x, na.y), make_float2(na.z, na.w),
+                                   make_float2(nb.x, nb.y), make_float2(nb.z, nb.w)};
             const float base = fmaf(al, fx0, be * fy);
+            const float2 base2 = make_float2(base, base), al2 = make_float2(al, al), ga2 = make_float2(ga, ga);
+            const float2 m1 = make_float2(-1.f, -1.f);
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-              float sn, cs;
-              __sincosf(fmaf(ga, npv[j], fmaf(al, static_cast<float>(j), base)), &sn, &cs);
-              const float ch = dtc_head(cs), sh = dtc_head(sn);
-              hi[2 * j] = __float_as_uint(ch);
-              hi[2 * j + 1] = __float_as_uint(sh);
-              lo[2 * j] = __float_as_uint(cs - ch);
-              lo[2 * j + 1] = __float_as_uint(sn - sh);
+            for (int j2 = 0; j2 < 4; ++j2) {
+              // two pixels per packed FFMA; (cos, sin) pairs split by one packed FFMA each
+              const float2 jj = make_float2(static_cast<float>(2 * j2), static_cast<float>(2 * j2 + 1));
+              const float2 ph = ffma2(ga2, np2[j2], ffma2(al2, jj, base2));
+              float2 e0, e1;                            // (cos, sin) of the two phases
+              __sincosf(ph.x, &e0.y, &e0.x);
+              __sincosf(ph.y, &e1.y, &e1.x);
+              const float2 h0 = make_float2(dtc_head(e0.x), dtc_head(e0.y));
+              const float2 h1 = make_float2(dtc_head(e1.x), dtc_head(e1.y));
+              const float2 l0 = ffma2(h0, m1, e0), l1 = ffma2(h1, m1, e1);          // e - head, exact
+              hi[4 * j2] = __float_as_uint(h0.x);
+              hi[4 * j2 + 1] = __float_as_uint(h0.y);
+              hi[4 * j2 + 2] = __float_as_uint(h1.x);
+              hi[4 * j2 + 3] = __float_as_uint(h1.y);
+              lo[4 * j2] = __float_as_uint(l0.x);
+              lo[4 * j2 + 1] = __float_as_uint(l0.y);
+              lo[4 * j2 + 2] = __float_as_uint(l1.x);
+              lo[4 * j2 + 3] = __float_as_uint(l1.y);
             }
           }
           // the previous slot: its stores finished long ago
@@ -317,7 +344,7 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + 32, 1)
             np_addr += kKC * 4;
             fx0 += static_cast<float>(kKC);
             if (fx0 >= static_cast<float>(L / 2)) { fx0 = static_cast<float>(-L / 2); fy += 1.f; }
-            if (++cl == ncs) { cl = 0; ++st; }
+            --cl;
           }
         }
         pending = true;
@@ -370,7 +397,7 @@ cudaError_t launch(const SubgridJob& job, const float2* in, float4* vis, cudaStr
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  kernel<<<static_cast<unsigned>(job.count), NG * kTileV + NG * 32 + 32, dyn, stream>>>(job, in, vis);
+  kernel<<<static_cast<unsigned>(job.count), NG * kTileV + NG * 32 + kProducers * 32, dyn, stream>>>(job, in, vis);
   count_launch();
   return cudaGetLastError();
 }

@@ -334,16 +334,27 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, 1)
               for (int half = 0; half < KC / 8; ++half) {
                 const float4 dka = tc::lds128(dk_addr + half * 32);
                 const float4 dkb = tc::lds128(dk_addr + half * 32 + 16);
-                const float dk[8] = {dka.x, dka.y, dka.z, dka.w, dkb.x, dkb.y, dkb.z, dkb.w};
+                const float2 dk2[4] = {make_float2(dka.x, dka.y), make_float2(dka.z, dka.w),
+                                       make_float2(dkb.x, dkb.y), make_float2(dkb.z, dkb.w)};
+                const float2 pa2 = make_float2(pa, pa), pb2 = make_float2(pb, pb), m1 = make_float2(-1.f, -1.f);
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                  float sn, cs;
-                  __sincosf(fmaf(pa, dk[j], pb), &sn, &cs);
-                  const float ch = tf32_head(cs), sh = tf32_head(sn);
-                  hi[half][2 * j] = __float_as_uint(ch);
-                  hi[half][2 * j + 1] = __float_as_uint(sh);
-                  lo[half][2 * j] = __float_as_uint(cs - ch);
-                  lo[half][2 * j + 1] = __float_as_uint(sn - sh);
+                for (int j2 = 0; j2 < 4; ++j2) {
+                  // two visibilities per packed FFMA; (cos, sin) pairs split by one packed FFMA each
+                  const float2 ph = ffma2(pa2, dk2[j2], pb2);
+                  float2 e0, e1;                        // (cos, sin) of the two phases
+                  __sincosf(ph.x, &e0.y, &e0.x);
+                  __sincosf(ph.y, &e1.y, &e1.x);
+                  const float2 h0 = make_float2(tf32_head(e0.x), tf32_head(e0.y));
+                  const float2 h1 = make_float2(tf32_head(e1.x), tf32_head(e1.y));
+                  const float2 l0 = ffma2(h0, m1, e0), l1 = ffma2(h1, m1, e1);      // e - head, exact
+                  hi[half][4 * j2] = __float_as_uint(h0.x);
+                  hi[half][4 * j2 + 1] = __float_as_uint(h0.y);
+                  hi[half][4 * j2 + 2] = __float_as_uint(h1.x);
+                  hi[half][4 * j2 + 3] = __float_as_uint(h1.y);
+                  lo[half][4 * j2] = __float_as_uint(l0.x);
+                  lo[half][4 * j2 + 1] = __float_as_uint(l0.y);
+                  lo[half][4 * j2 + 2] = __float_as_uint(l1.x);
+                  lo[half][4 * j2 + 3] = __float_as_uint(l1.y);
                 }
               }
             }
