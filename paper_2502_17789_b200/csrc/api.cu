@@ -73,11 +73,26 @@ cudaError_t upload_csr(const TileCsr& csr, DeviceCsr* out) {
   cudaError_t e;
   if ((e = upload(csr.tile_ids, &out->tile_ids)) != cudaSuccess) return e;
   if ((e = upload(csr.offsets, &out->offsets)) != cudaSuccess) return e;
-  return upload(csr.items, &out->items);
+  if ((e = upload(csr.items, &out->items)) != cudaSuccess) return e;
+  out->n_segs = static_cast<int32_t>(csr.segs.size() / kSegStride);
+  out->n_slots = csr.n_slots;
+  return upload(csr.segs, &out->segs);
+}
+
+// fp64 partial sums [n_slots][4 pol][kTile][kTile][re, im] and one zeroed counter per tile
+constexpr size_t kPartialBytes = static_cast<size_t>(4) * kTile * kTile * 2 * sizeof(double);
+cudaError_t alloc_adder_scratch(int32_t n_slots, int32_t n_tiles, double** partials, int32_t** counters) {
+  *partials = nullptr; *counters = nullptr;
+  if (n_slots == 0) return cudaSuccess;
+  cudaError_t e = cudaMalloc(reinterpret_cast<void**>(partials), kPartialBytes * n_slots);
+  if (e != cudaSuccess) return e;
+  e = cudaMalloc(reinterpret_cast<void**>(counters), sizeof(int32_t) * n_tiles);
+  if (e != cudaSuccess) return e;
+  return cudaMemset(*counters, 0, sizeof(int32_t) * n_tiles);
 }
 
 void free_csr(DeviceCsr* c) {
-  cudaFree(c->tile_ids); cudaFree(c->offsets); cudaFree(c->items);
+  cudaFree(c->tile_ids); cudaFree(c->offsets); cudaFree(c->items); cudaFree(c->segs);
   *c = DeviceCsr{};
 }
 
@@ -85,6 +100,7 @@ void free_device_state(DeviceState* d) {
   if (!d) return;
   cudaFree(d->uvw); cudaFree(d->kappa); cudaFree(d->meta); cudaFree(d->nprime);
   for (auto& c : d->batch_csr) free_csr(&c);
+  cudaFree(d->adder_partials); cudaFree(d->adder_counters);
   delete d;
 }
 
@@ -128,6 +144,14 @@ int ensure_device(const idg_plan* plan, const DeviceState** out) {
       return cuda_fail(e, "plan upload (tile lists)");
     }
   }
+  // the adder's scratch is shared by the batches (they run one after another on one stream)
+  int32_t max_slots = 0, max_tiles = 0;
+  for (const auto& c : d->batch_csr) { max_slots = std::max(max_slots, c.n_slots); max_tiles = std::max(max_tiles, c.n_tiles); }
+  if ((e = alloc_adder_scratch(max_slots, max_tiles, &d->adder_partials, &d->adder_counters)) != cudaSuccess) {
+    free_device_state(d);
+    return cuda_fail(e, "plan upload (adder scratch)");
+  }
+  for (auto& c : d->batch_csr) { c.partials = d->adder_partials; c.counters = d->adder_counters; }
   plan->dev = d;
   *out = d;
   return IDG_OK;
@@ -492,10 +516,12 @@ int idg_adder(const idg_plan* plan, int64_t first, int64_t count, const void* su
   build_tile_csr(plan, first, count, &csr);
   DeviceCsr dc;
   cudaError_t e = upload_csr(csr, &dc);
-  if (e != cudaSuccess) { free_csr(&dc); return cuda_fail(e, "idg_adder: tile list upload"); }
+  if (e == cudaSuccess) e = alloc_adder_scratch(dc.n_slots, dc.n_tiles, &dc.partials, &dc.counters);
+  if (e != cudaSuccess) { cudaFree(dc.partials); cudaFree(dc.counters); free_csr(&dc); return cuda_fail(e, "idg_adder: tile list upload"); }
   e = launch_adder(d->meta, dc, first, plan->par.subgrid_size, plan->par.grid_size, plan->tiles_x, plan->tiles_y,
                    static_cast<const float2*>(subgrids_dev), static_cast<float2*>(grid_dev), stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+  cudaFree(dc.partials); cudaFree(dc.counters);
   free_csr(&dc);
   if (e != cudaSuccess) return cuda_fail(e, "idg_adder");
   return IDG_OK;

@@ -13,19 +13,29 @@ namespace idg {
 constexpr double kSpeedOfLight = 299792458.0;
 constexpr int kMetaStride = 12;   // int32 per subgrid on the device: b,t0,nt,c0,nc,x0,y0,wl,p,q,it,layer
 constexpr int kTile = 32;         // adder tile edge in master-grid pixels
+constexpr int kAdderSegment = 128;   // subgrids one adder block walks; longer tile lists are split
+constexpr int kSegStride = 6;     // int32 per adder segment: tile index, begin, end, k, n_seg, partial slot
 
 // tile -> subgrid lists for the atomic-free adder (one CSR per batch of subgrids).
 struct TileCsr {
   std::vector<int32_t> tile_ids;   // (layer*tiles_y + ty)*tiles_x + tx of every non-empty tile
   std::vector<int32_t> offsets;    // [n_tiles + 1] into items
   std::vector<int32_t> items;      // subgrid indices (global), ascending within a tile
+  // Work units of the adder: segment k of n_seg of a tile's list, items [begin, end).  A tile with one
+  // segment is added to the grid directly; otherwise every segment leaves an fp64 partial sum in
+  // `slot` and the tile's last block to finish adds them up in the order k = 0, 1, ... (fixed order).
+  std::vector<int32_t> segs;       // [n_segs, kSegStride], longest first
+  int32_t n_slots = 0;
 };
 
 struct DeviceCsr {
   int32_t* tile_ids = nullptr;
   int32_t* offsets = nullptr;
   int32_t* items = nullptr;
-  int32_t n_tiles = 0;
+  int32_t* segs = nullptr;
+  int32_t n_tiles = 0, n_segs = 0, n_slots = 0;
+  double* partials = nullptr;      // [n_slots, 4, kTile, kTile, 2] scratch (not owned: DeviceState / caller)
+  int32_t* counters = nullptr;     // [n_tiles] segments finished per tile, zero between launches
 };
 
 struct Batch {
@@ -39,6 +49,8 @@ struct DeviceState {
   int32_t* meta = nullptr;      // [n_subgrids, kMetaStride]
   float* nprime = nullptr;      // [L, L] n'(l, m) at the subgrid pixels
   std::vector<DeviceCsr> batch_csr;
+  double* adder_partials = nullptr;   // shared by the batches: sized for the largest
+  int32_t* adder_counters = nullptr;
   int device = -1;
 };
 

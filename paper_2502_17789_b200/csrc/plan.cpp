@@ -185,6 +185,25 @@ void build_tile_csr(const idg_plan* plan, int64_t first, int64_t count, TileCsr*
     for (size_t i = r.beg; i < r.end; ++i) out->items.push_back(pairs[i].second);
   }
   out->offsets.push_back(static_cast<int32_t>(out->items.size()));
+  // segments: a block walks at most kAdderSegment subgrids, so one dense tile does not serialise the launch
+  struct Seg { int32_t tile, beg, end, k, n, slot; };
+  std::vector<Seg> segs;
+  out->n_slots = 0;
+  for (size_t t = 0; t < out->tile_ids.size(); ++t) {
+    const int32_t beg = out->offsets[t], end = out->offsets[t + 1];
+    const int32_t n = (end - beg + kAdderSegment - 1) / kAdderSegment;
+    for (int32_t k = 0; k < n; ++k) {
+      const int32_t b = beg + k * kAdderSegment, e = std::min(end, b + kAdderSegment);
+      segs.push_back({static_cast<int32_t>(t), b, e, k, n, n > 1 ? out->n_slots++ : -1});
+    }
+  }
+  std::stable_sort(segs.begin(), segs.end(), [](const Seg& a, const Seg& b) { return (a.end - a.beg) > (b.end - b.beg); });
+  out->segs.clear();
+  out->segs.reserve(segs.size() * kSegStride);
+  for (const Seg& g : segs) {
+    const int32_t rec[kSegStride] = {g.tile, g.beg, g.end, g.k, g.n, g.slot};
+    out->segs.insert(out->segs.end(), rec, rec + kSegStride);
+  }
 }
 
 // Per-subgrid device metadata: the 8 plan fields plus stations (p, q), A-term interval and
