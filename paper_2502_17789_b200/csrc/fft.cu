@@ -1,163 +1,231 @@
-// Subgrid FFT: steps a4 / a7.  Centred L x L DFT of one plane per block, in shared memory,
-// scaled by 1/L^2 (Eq. 7-8 :107-117, :157, :170; R1, R2).
+// Subgrid FFT: steps a4 / a7.  Centred L x L DFT of one plane per block, scaled by 1/L^2
+// (Eq. 7-8 :107-117, :157, :170; R1, R2).
 //
-// For L a multiple of 4 the centred transform equals checkerboard * FFT * checkerboard
-// ((-1)^(x+y) on input and output), so the kernel is a plain in-place mixed-radix
-// decimation-in-time FFT: the load from global memory applies the checkerboard and the
-// digit-reversal permutation of both axes, the row and column passes then run in place with
-// radix-4/2/3 butterflies, and the store applies the checkerboard and the 1/L^2.
+// For even L the centred transform equals checkerboard * DFT * checkerboard ((-1)^(x+y) on input and
+// output), so the kernel is a plain 2-D FFT with the checkerboard folded into the global load and
+// the checkerboard and 1/L^2 into the global store.
+//
+// Every 1-D transform of length L = 8 R2 (R2 = 4, 8, 12, 16) is two register-resident steps:
+//   n = n1 R2 + n2, k = k1 + 8 k2:
+//   step 1  Y[k1][n2] = w_L^(n2 k1) * sum_n1 x[n1 R2 + n2] w_8^(n1 k1)     (radix-8 butterfly per n2)
+//   step 2  X[k1 + 8 k2] = sum_n2 Y[k1][n2] w_R2^(n2 k2)                   (radix-R2 butterfly per k1)
+// A plane therefore makes one trip global -> registers (row step 1) -> shared -> registers (row step
+// 2) -> shared -> registers (column step 1, in place) -> shared -> registers (column step 2) -> global:
+// three shared-memory round trips and three block barriers, against one round trip per radix-4 stage
+// before.  Row step 2 is the only step whose tasks read and write different positions of a line; a
+// warp owns whole rows there, so a warp-level barrier between its reads and writes is enough.
 #include "kernels.h"
 
 namespace idg {
 
 namespace {
 
-// radix of stage s (stage 0 first, sub-transform size 1) for each supported L
-template <int L>
-__host__ __device__ constexpr int radix(int s) {
-  return L == 32   ? (s < 2 ? 4 : (s == 2 ? 2 : 1))
-         : L == 64 ? (s < 3 ? 4 : 1)
-         : L == 96 ? (s < 2 ? 4 : (s == 2 ? 2 : (s == 3 ? 3 : 1)))
-                   : (s < 3 ? 4 : (s == 3 ? 2 : 1));
-}
-template <int L>
-__host__ __device__ constexpr int n_stages() { return (L == 32 || L == 64) ? 3 : 4; }
-
-// position of natural index n in the digit-reversed input order of the in-place DIT:
-// pos_N(n) = (n mod r_k) * N_{k-1} + pos_{N_{k-1}}(n div r_k), r_k the radix of the last stage.
-template <int L>
-__host__ __device__ constexpr int dit_position(int n) {
-  int pos = 0;
-  int size = L;
-  for (int s = n_stages<L>() - 1; s >= 0; --s) {
-    const int r = radix<L>(s);
-    size /= r;
-    pos += (n % r) * size;
-    n /= r;
-  }
-  return pos;
-}
-
+__device__ __forceinline__ float2 cadd2(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub2(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
 __device__ __forceinline__ float2 cmulf(float2 a, float2 b) {
   return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
 }
-
-// One radix-R DIT stage over `lines` independent length-L lines.  Element e of line q lives at
-// data[q * line_stride + e * elem_stride].  m = product of the radices already done.
-// tw[k] = exp(-+ 2 pi i k / L).  SIGN = -1 forward, +1 inverse.
-template <int L, int R, int M, int SIGN, int T>
-__device__ __forceinline__ void fft_stage(float2* data, const float2* tw, int line_stride, int elem_stride) {
-  constexpr int m = M;
-  constexpr int BF = L / R;              // butterflies per line
-  const int total = BF * L;              // L lines
-  for (int idx = threadIdx.x; idx < total; idx += T) {
-    const int line = idx % L, bf = idx / L;   // consecutive threads take consecutive lines
-    const int j = bf % m;
-    const int blk = bf / m;
-    float2* p = data + line * line_stride + (blk * m * R + j) * elem_stride;
-    const int tstep = j * (L / (m * R));   // twiddle index step: w_{mR}^{j q} = tw[j q L/(mR)]
-    float2 x[R];
-#pragma unroll
-    for (int q = 0; q < R; ++q) {
-      x[q] = p[q * m * elem_stride];
-      if (q > 0) x[q] = cmulf(x[q], tw[q * tstep]);
-    }
-    if (R == 2) {
-      const float2 a = x[0], b = x[1];
-      x[0] = make_float2(a.x + b.x, a.y + b.y);
-      x[1] = make_float2(a.x - b.x, a.y - b.y);
-    } else if (R == 4) {
-      const float2 s02 = make_float2(x[0].x + x[2].x, x[0].y + x[2].y);
-      const float2 d02 = make_float2(x[0].x - x[2].x, x[0].y - x[2].y);
-      const float2 s13 = make_float2(x[1].x + x[3].x, x[1].y + x[3].y);
-      const float2 d13 = make_float2(x[1].x - x[3].x, x[1].y - x[3].y);
-      // SIGN*i * d13 : forward (-i): (d.y, -d.x); inverse (+i): (-d.y, d.x)
-      const float2 r13 = SIGN < 0 ? make_float2(d13.y, -d13.x) : make_float2(-d13.y, d13.x);
-      x[0] = make_float2(s02.x + s13.x, s02.y + s13.y);
-      x[1] = make_float2(d02.x + r13.x, d02.y + r13.y);
-      x[2] = make_float2(s02.x - s13.x, s02.y - s13.y);
-      x[3] = make_float2(d02.x - r13.x, d02.y - r13.y);
-    } else if (R == 3) {
-      // y0 = x0+x1+x2; y1 = x0 + w x1 + w^2 x2; y2 = x0 + w^2 x1 + w x2, w = exp(SIGN 2 pi i/3)
-      const float hs = SIGN * 0.86602540378443864676f;   // Im(w)
-      const float2 s = make_float2(x[1].x + x[2].x, x[1].y + x[2].y);
-      const float2 d = make_float2(x[1].x - x[2].x, x[1].y - x[2].y);
-      const float2 c = make_float2(fmaf(-0.5f, s.x, x[0].x), fmaf(-0.5f, s.y, x[0].y));
-      // i*hs*d = (-hs d.y, hs d.x)
-      const float2 e = make_float2(-hs * d.y, hs * d.x);
-      x[0] = make_float2(x[0].x + s.x, x[0].y + s.y);
-      x[1] = make_float2(c.x + e.x, c.y + e.y);
-      x[2] = make_float2(c.x - e.x, c.y - e.y);
-    }
-#pragma unroll
-    for (int q = 0; q < R; ++q) p[q * m * elem_stride] = x[q];
+// multiply by SIGN * i  (forward: -i)
+template <int SIGN>
+__device__ __forceinline__ float2 rot90(float2 d) {
+  return SIGN < 0 ? make_float2(d.y, -d.x) : make_float2(-d.y, d.x);
+}
+// exp(SIGN 2 pi i m / N) for the small transforms; the tables fold to immediates once unrolled
+template <int N, int SIGN>
+__device__ __forceinline__ float2 wsmall(int m) {
+  if constexpr (N == 8) {
+    const float c[8] = {1.f, 0.707106781f, 0.f, -0.707106781f, -1.f, -0.707106781f, 0.f, 0.707106781f};
+    const float s[8] = {0.f, 0.707106781f, 1.f, 0.707106781f, 0.f, -0.707106781f, -1.f, -0.707106781f};
+    return make_float2(c[m], SIGN * s[m]);
+  } else if constexpr (N == 12) {
+    const float c[12] = {1.f, 0.866025404f, 0.5f, 0.f, -0.5f, -0.866025404f, -1.f, -0.866025404f, -0.5f, 0.f, 0.5f,
+                         0.866025404f};
+    const float s[12] = {0.f, 0.5f, 0.866025404f, 1.f, 0.866025404f, 0.5f, 0.f, -0.5f, -0.866025404f, -1.f,
+                         -0.866025404f, -0.5f};
+    return make_float2(c[m], SIGN * s[m]);
+  } else {
+    const float c[16] = {1.f, 0.923879533f, 0.707106781f, 0.382683432f, 0.f, -0.382683432f, -0.707106781f,
+                         -0.923879533f, -1.f, -0.923879533f, -0.707106781f, -0.382683432f, 0.f, 0.382683432f,
+                         0.707106781f, 0.923879533f};
+    const float s[16] = {0.f, 0.382683432f, 0.707106781f, 0.923879533f, 1.f, 0.923879533f, 0.707106781f,
+                         0.382683432f, 0.f, -0.382683432f, -0.707106781f, -0.923879533f, -1.f, -0.923879533f,
+                         -0.707106781f, -0.382683432f};
+    return make_float2(c[m], SIGN * s[m]);
   }
 }
 
-template <int L, int SIGN, int T, int S, int M>
-struct Pass {
-  static __device__ __forceinline__ void run(float2* data, const float2* tw, int line_stride, int elem_stride) {
-    constexpr int R = radix<L>(S);
-    fft_stage<L, R, M, SIGN, T>(data, tw, line_stride, elem_stride);
-    __syncthreads();
-    Pass<L, SIGN, T, S + 1, M * R>::run(data, tw, line_stride, elem_stride);
+// ---- small DFTs on registers, natural order in and out: X[k] = sum_n x[n] exp(SIGN 2 pi i n k / N)
+template <int SIGN>
+__device__ __forceinline__ void dft2(float2& a, float2& b) {
+  const float2 s = cadd2(a, b), d = csub2(a, b);
+  a = s; b = d;
+}
+template <int SIGN>
+__device__ __forceinline__ void dft3(float2& x0, float2& x1, float2& x2) {
+  const float hs = SIGN * 0.86602540378443864676f;   // Im exp(SIGN 2 pi i / 3)
+  const float2 s = cadd2(x1, x2), d = csub2(x1, x2);
+  const float2 c = make_float2(fmaf(-0.5f, s.x, x0.x), fmaf(-0.5f, s.y, x0.y));
+  const float2 e = make_float2(-hs * d.y, hs * d.x);  // i hs d
+  x0 = cadd2(x0, s); x1 = cadd2(c, e); x2 = csub2(c, e);
+}
+template <int SIGN>
+__device__ __forceinline__ void dft4(float2& x0, float2& x1, float2& x2, float2& x3) {
+  const float2 a = cadd2(x0, x2), b = csub2(x0, x2), c = cadd2(x1, x3), d = rot90<SIGN>(csub2(x1, x3));
+  x0 = cadd2(a, c); x1 = cadd2(b, d); x2 = csub2(a, c); x3 = csub2(b, d);
+}
+// N = P Q by the same index split as above: n = n1 Q + n2, k = k1 + P k2
+template <int N, int SIGN>
+__device__ __forceinline__ void dft_small(float2 (&x)[N]) {
+  if constexpr (N == 4) {
+    dft4<SIGN>(x[0], x[1], x[2], x[3]);
+  } else {
+    constexpr int P = 4, Q = N / 4;                  // 8 = 4 x 2, 12 = 4 x 3, 16 = 4 x 4
+    float2 y[N];                                     // y[k1 * Q + n2]
+#pragma unroll
+    for (int n2 = 0; n2 < Q; ++n2) {
+      float2 a = x[n2], b = x[Q + n2], c = x[2 * Q + n2], d = x[3 * Q + n2];
+      dft4<SIGN>(a, b, c, d);
+      y[n2] = a;
+      y[Q + n2] = n2 ? cmulf(b, wsmall<N, SIGN>(n2)) : b;
+      y[2 * Q + n2] = n2 ? cmulf(c, wsmall<N, SIGN>(2 * n2)) : c;
+      y[3 * Q + n2] = n2 ? cmulf(d, wsmall<N, SIGN>(3 * n2)) : d;
+    }
+#pragma unroll
+    for (int k1 = 0; k1 < P; ++k1) {
+      if constexpr (Q == 2) {
+        dft2<SIGN>(y[k1 * Q], y[k1 * Q + 1]);
+      } else if constexpr (Q == 3) {
+        dft3<SIGN>(y[k1 * Q], y[k1 * Q + 1], y[k1 * Q + 2]);
+      } else {
+        dft4<SIGN>(y[k1 * Q], y[k1 * Q + 1], y[k1 * Q + 2], y[k1 * Q + 3]);
+      }
+#pragma unroll
+      for (int k2 = 0; k2 < Q; ++k2) x[k1 + P * k2] = y[k1 * Q + k2];
+    }
   }
-};
-template <int L, int SIGN, int T, int S>
-struct Pass<L, SIGN, T, S, L> {
-  static __device__ __forceinline__ void run(float2*, const float2*, int, int) {}
-};
+}
 
-template <int L, int SIGN, int T>
-__global__ void __launch_bounds__(T) fft_kernel(float2* __restrict__ planes) {
-  constexpr int PITCH = L + 1;
+template <int L>
+struct FftThreads { static constexpr int value = L == 32 ? 128 : (L == 64 ? 256 : (L == 96 ? 576 : 512)); };
+
+template <int L, int SIGN>
+__global__ void __launch_bounds__(FftThreads<L>::value) fft_kernel(float2* __restrict__ planes) {
+  constexpr int T = FftThreads<L>::value;
+  constexpr int R2 = L / 8;
+  constexpr int PITCH = L + 9;                       // row step 1 stores 8 groups of R2 + 1 (conflict-free reads)
+  static_assert(R2 == 4 || R2 == 8 || R2 == 12 || R2 == 16, "L = 8 R2");
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float2* data = reinterpret_cast<float2*>(smem_raw);          // [L][PITCH]
-  float2* tw = data + L * PITCH;                               // [L]
-  int* pos = reinterpret_cast<int*>(tw + L);                   // [L]
+  float2* tw = data + L * PITCH;                               // [L] exp(SIGN 2 pi i m / L)
   float2* plane = planes + static_cast<int64_t>(blockIdx.x) * L * L;
+  const int tid = threadIdx.x;
 
-  for (int k = threadIdx.x; k < L; k += T) {
+  for (int k = tid; k < L; k += T) {
     float s, c;
     sincospif(2.0f * k / L, &s, &c);
     tw[k] = make_float2(c, SIGN * s);
-    pos[k] = dit_position<L>(k);
+  }
+
+  // ---- rows, step 1: global -> radix-8 over n1 -> twiddle -> shared [r][k1 (R2 + 1) + n2]
+  // (the twiddle table is read only after the barrier below, so step 1 is split around it)
+  constexpr int IT_R1 = (L * R2 + T - 1) / T;
+  float2 xr[IT_R1][8];
+#pragma unroll
+  for (int it = 0; it < IT_R1; ++it) {
+    const int t = tid + it * T, r = t / R2, n2 = t % R2;
+    if (t < L * R2) {
+      const float sg = ((r + n2) & 1) ? -1.f : 1.f;   // checkerboard; R2 is even, so n1 R2 drops out
+#pragma unroll
+      for (int n1 = 0; n1 < 8; ++n1) {
+        const float2 v = plane[r * L + n1 * R2 + n2];
+        xr[it][n1] = make_float2(v.x * sg, v.y * sg);
+      }
+      dft_small<8, SIGN>(xr[it]);
+    }
+  }
+  __syncthreads();                                    // twiddles ready
+#pragma unroll
+  for (int it = 0; it < IT_R1; ++it) {
+    const int t = tid + it * T, r = t / R2, n2 = t % R2;
+    if (t < L * R2) {
+      float2* row = data + r * PITCH + n2;
+      row[0] = xr[it][0];
+#pragma unroll
+      for (int k1 = 1; k1 < 8; ++k1) row[k1 * (R2 + 1)] = cmulf(xr[it][k1], tw[n2 * k1]);
+    }
   }
   __syncthreads();
-  for (int i = threadIdx.x; i < L * L; i += T) {
-    const int y = i / L, x = i % L;
-    float2 v = plane[i];
-    if ((x + y) & 1) v = make_float2(-v.x, -v.y);
-    data[pos[y] * PITCH + pos[x]] = v;
+
+  // ---- rows, step 2: a warp owns 4 whole rows; read, warp barrier, radix-R2 over n2, write natural order
+  constexpr int IT_R2 = (L * 8 + T - 1) / T;
+#pragma unroll
+  for (int it = 0; it < IT_R2; ++it) {
+    const int t = tid + it * T, r = t >> 3, k1 = t & 7;
+    if (t < L * 8) {                                  // warp-uniform: T and 8 L are multiples of 32
+      float2 y[R2];
+      const float2* src = data + r * PITCH + k1 * (R2 + 1);
+#pragma unroll
+      for (int n2 = 0; n2 < R2; ++n2) y[n2] = src[n2];
+      __syncwarp();
+      dft_small<R2, SIGN>(y);
+      float2* dst = data + r * PITCH + k1;
+#pragma unroll
+      for (int k2 = 0; k2 < R2; ++k2) dst[8 * k2] = y[k2];
+    }
   }
   __syncthreads();
-  // rows: element stride 1, lines = rows; consecutive threads take consecutive rows
-  Pass<L, SIGN, T, 0, 1>::run(data, tw, PITCH, 1);
-  // columns: element stride PITCH, lines = columns; consecutive threads take consecutive columns
-  Pass<L, SIGN, T, 0, 1>::run(data, tw, 1, PITCH);
+
+  // ---- columns, step 1 (in place): radix-8 over n1, twiddle; consecutive threads = consecutive columns
+  constexpr int IT_C1 = (L * R2 + T - 1) / T;
+#pragma unroll
+  for (int it = 0; it < IT_C1; ++it) {
+    const int t = tid + it * T, n2 = t / L, c = t % L;
+    if (t < L * R2) {
+      float2 x[8];
+      float2* col = data + n2 * PITCH + c;
+#pragma unroll
+      for (int n1 = 0; n1 < 8; ++n1) x[n1] = col[n1 * R2 * PITCH];
+      dft_small<8, SIGN>(x);
+      col[0] = x[0];
+#pragma unroll
+      for (int k1 = 1; k1 < 8; ++k1) col[k1 * R2 * PITCH] = cmulf(x[k1], tw[n2 * k1]);
+    }
+  }
+  __syncthreads();
+
+  // ---- columns, step 2: radix-R2 over n2 -> checkerboard, 1/L^2 -> global (rows of 8 L bytes, coalesced)
+  constexpr int IT_C2 = (L * 8 + T - 1) / T;
   const float scale = 1.0f / (L * L);
-  for (int i = threadIdx.x; i < L * L; i += T) {
-    const int y = i / L, x = i % L;
-    float2 v = data[y * PITCH + x];
-    const float sc = ((x + y) & 1) ? -scale : scale;
-    plane[i] = make_float2(v.x * sc, v.y * sc);
+#pragma unroll
+  for (int it = 0; it < IT_C2; ++it) {
+    const int t = tid + it * T, k1 = t / L, c = t % L;
+    if (t < L * 8) {
+      float2 y[R2];
+      const float2* col = data + k1 * R2 * PITCH + c;
+#pragma unroll
+      for (int n2 = 0; n2 < R2; ++n2) y[n2] = col[n2 * PITCH];
+      dft_small<R2, SIGN>(y);
+      const float sc = ((k1 + c) & 1) ? -scale : scale;   // 8 k2 is even
+#pragma unroll
+      for (int k2 = 0; k2 < R2; ++k2) plane[(k1 + 8 * k2) * L + c] = make_float2(y[k2].x * sc, y[k2].y * sc);
+    }
   }
 }
 
 template <int L>
 cudaError_t launch(int64_t n_planes, float2* planes, int direction, cudaStream_t stream) {
-  constexpr int T = 256;
-  const size_t smem = static_cast<size_t>(L) * (L + 1) * sizeof(float2) + L * sizeof(float2) + L * sizeof(int);
+  constexpr int T = FftThreads<L>::value;
+  const size_t smem = static_cast<size_t>(L) * (L + 9) * sizeof(float2) + L * sizeof(float2);
   if (n_planes == 0) return cudaSuccess;
   cudaError_t e;
   if (direction > 0) {
-    e = cudaFuncSetAttribute(fft_kernel<L, -1, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+    e = cudaFuncSetAttribute(fft_kernel<L, -1>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
     if (e != cudaSuccess) return e;
-    fft_kernel<L, -1, T><<<static_cast<unsigned>(n_planes), T, smem, stream>>>(planes);
+    fft_kernel<L, -1><<<static_cast<unsigned>(n_planes), T, smem, stream>>>(planes);
   } else {
-    e = cudaFuncSetAttribute(fft_kernel<L, +1, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+    e = cudaFuncSetAttribute(fft_kernel<L, +1>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
     if (e != cudaSuccess) return e;
-    fft_kernel<L, +1, T><<<static_cast<unsigned>(n_planes), T, smem, stream>>>(planes);
+    fft_kernel<L, +1><<<static_cast<unsigned>(n_planes), T, smem, stream>>>(planes);
   }
   count_launch();
   return cudaGetLastError();
