@@ -1,6 +1,7 @@
 // C-ABI layer: argument validation, plan lifetime, lazy upload of the plan metadata, and the
 // orchestration of the kernels per batch.  See include/idg_b200.h for the contract.
 #include <atomic>
+#include <functional>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -318,6 +319,45 @@ size_t idg_workspace_bytes(const idg_plan* plan, int direction) {
   return stack_bytes(plan, plan->batch_capacity);
 }
 
+namespace {
+
+// One batch of the imaging direction: gridder, subgrid FFT, adder.  `before_adder` runs on the host
+// between the FFT and the adder launches (the host-buffer call waits for the grid upload there).
+int grid_batch(const idg_plan* plan, const DeviceState* d, size_t i, const void* vis_dev, const void* aterms_dev,
+               const float* taper_dev, void* grid_dev, float2* stack, cudaStream_t stream,
+               const std::function<int()>& before_adder) {
+  const int L = plan->par.subgrid_size, Ng = plan->par.grid_size;
+  const Batch& bt = plan->batches[i];
+  const SubgridJob job = make_job(plan, d, bt.first, bt.count, aterms_dev, taper_dev);
+  { ProfScope ps(IDG_K_GRIDDER, stream);
+    IDG_CUDA(run_gridder(plan, job, static_cast<const float4*>(vis_dev), stack, stream)); }
+  { ProfScope ps(IDG_K_FFT, stream);
+    IDG_CUDA(launch_subgrid_fft(L, bt.count * 4, stack, +1, stream)); }
+  int rc = before_adder();
+  if (rc != IDG_OK) return rc;
+  { ProfScope ps(IDG_K_ADDER, stream);
+    IDG_CUDA(launch_adder(d->meta, d->batch_csr[i], bt.first, L, Ng, plan->tiles_x, plan->tiles_y, stack,
+                          static_cast<float2*>(grid_dev), stream)); }
+  return IDG_OK;
+}
+
+// One batch of the prediction direction: splitter, inverse subgrid FFT, degridder.
+int degrid_batch(const idg_plan* plan, const DeviceState* d, size_t i, const void* grid_dev, const void* aterms_dev,
+                 const float* taper_dev, void* vis_dev, float2* stack, cudaStream_t stream) {
+  const int L = plan->par.subgrid_size, Ng = plan->par.grid_size;
+  const Batch& bt = plan->batches[i];
+  const SubgridJob job = make_job(plan, d, bt.first, bt.count, aterms_dev, taper_dev);
+  { ProfScope ps(IDG_K_SPLITTER, stream);
+    IDG_CUDA(launch_splitter(d->meta, bt.first, bt.count, L, Ng, static_cast<const float2*>(grid_dev), stack, stream)); }
+  { ProfScope ps(IDG_K_IFFT, stream);
+    IDG_CUDA(launch_subgrid_fft(L, bt.count * 4, stack, -1, stream)); }
+  { ProfScope ps(IDG_K_DEGRIDDER, stream);
+    IDG_CUDA(run_degridder(plan, job, stack, static_cast<float4*>(vis_dev), stream)); }
+  return IDG_OK;
+}
+
+}  // namespace
+
 int idg_grid(const idg_plan* plan, const void* vis_dev, const void* aterms_dev, const float* taper_dev,
              void* grid_dev, void* workspace_dev, size_t workspace_bytes, void* cuda_stream) {
   if (!plan || !vis_dev || !aterms_dev || !taper_dev || !grid_dev) { set_error("idg_grid: null argument"); return IDG_EINVAL; }
@@ -330,18 +370,10 @@ int idg_grid(const idg_plan* plan, const void* vis_dev, const void* aterms_dev, 
   int rc = ensure_device(plan, &d);
   if (rc != IDG_OK) return rc;
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-  float2* stack = static_cast<float2*>(workspace_dev);
-  const int L = plan->par.subgrid_size, Ng = plan->par.grid_size;
   for (size_t i = 0; i < plan->batches.size(); ++i) {
-    const Batch& bt = plan->batches[i];
-    const SubgridJob job = make_job(plan, d, bt.first, bt.count, aterms_dev, taper_dev);
-    { ProfScope ps(IDG_K_GRIDDER, stream);
-      IDG_CUDA(run_gridder(plan, job, static_cast<const float4*>(vis_dev), stack, stream)); }
-    { ProfScope ps(IDG_K_FFT, stream);
-      IDG_CUDA(launch_subgrid_fft(L, bt.count * 4, stack, +1, stream)); }
-    { ProfScope ps(IDG_K_ADDER, stream);
-      IDG_CUDA(launch_adder(d->meta, d->batch_csr[i], bt.first, L, Ng, plan->tiles_x, plan->tiles_y, stack,
-                            static_cast<float2*>(grid_dev), stream)); }
+    rc = grid_batch(plan, d, i, vis_dev, aterms_dev, taper_dev, grid_dev, static_cast<float2*>(workspace_dev), stream,
+                    [] { return IDG_OK; });
+    if (rc != IDG_OK) return rc;
   }
   return IDG_OK;
 }
@@ -358,17 +390,9 @@ int idg_degrid(const idg_plan* plan, const void* grid_dev, const void* aterms_de
   int rc = ensure_device(plan, &d);
   if (rc != IDG_OK) return rc;
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-  float2* stack = static_cast<float2*>(workspace_dev);
-  const int L = plan->par.subgrid_size, Ng = plan->par.grid_size;
   for (size_t i = 0; i < plan->batches.size(); ++i) {
-    const Batch& bt = plan->batches[i];
-    const SubgridJob job = make_job(plan, d, bt.first, bt.count, aterms_dev, taper_dev);
-    { ProfScope ps(IDG_K_SPLITTER, stream);
-      IDG_CUDA(launch_splitter(d->meta, bt.first, bt.count, L, Ng, static_cast<const float2*>(grid_dev), stack, stream)); }
-    { ProfScope ps(IDG_K_IFFT, stream);
-      IDG_CUDA(launch_subgrid_fft(L, bt.count * 4, stack, -1, stream)); }
-    { ProfScope ps(IDG_K_DEGRIDDER, stream);
-      IDG_CUDA(run_degridder(plan, job, stack, static_cast<float4*>(vis_dev), stream)); }
+    rc = degrid_batch(plan, d, i, grid_dev, aterms_dev, taper_dev, vis_dev, static_cast<float2*>(workspace_dev), stream);
+    if (rc != IDG_OK) return rc;
   }
   return IDG_OK;
 }
@@ -398,6 +422,66 @@ size_t idg_host_arena_bytes(const idg_plan* plan, int direction) {
   return arena_layout(plan).total;
 }
 
+namespace {
+
+// Rows of the visibility table grouped by the first and by the last batch that touches them, as runs of
+// consecutive rows: the host-buffer calls upload a row just before the first batch that reads it and
+// download it right after the last batch that writes it, while the other batches compute.
+void ensure_row_runs(const idg_plan* plan) {
+  std::lock_guard<std::mutex> lock(plan->mu);
+  if (!plan->rows_first.empty() || plan->batches.empty()) return;
+  const size_t nb = plan->batches.size();
+  std::vector<int32_t> first(plan->n_rows, -1), last(plan->n_rows, -1);
+  for (size_t i = 0; i < nb; ++i) {
+    const Batch& bt = plan->batches[i];
+    for (int64_t s = bt.first; s < bt.first + bt.count; ++s) {
+      const int32_t* m = &plan->sub[static_cast<size_t>(s) * 8];
+      const int64_t r0 = static_cast<int64_t>(m[0]) * plan->par.n_times + m[1];
+      for (int64_t r = r0; r < r0 + m[2]; ++r) {
+        if (first[r] < 0) first[r] = static_cast<int32_t>(i);
+        last[r] = static_cast<int32_t>(i);
+      }
+    }
+  }
+  auto runs = [&](const std::vector<int32_t>& tag, std::vector<std::vector<std::pair<int64_t, int64_t>>>* out) {
+    out->assign(nb, {});
+    for (int64_t r = 0; r < plan->n_rows;) {
+      int64_t e = r + 1;
+      while (e < plan->n_rows && tag[e] == tag[r]) ++e;
+      if (tag[r] >= 0) (*out)[tag[r]].emplace_back(r, e);
+      r = e;
+    }
+  };
+  runs(first, &plan->rows_first);
+  runs(last, &plan->rows_last);
+}
+
+// a second stream and the events that order it against the caller's stream; all destroyed on return
+struct CopyLane {
+  cudaStream_t s = nullptr;
+  std::vector<cudaEvent_t> ev;
+  ~CopyLane() {
+    for (cudaEvent_t e : ev) cudaEventDestroy(e);
+    if (s) cudaStreamDestroy(s);
+  }
+  cudaError_t init() { return cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking); }
+  cudaError_t event(cudaEvent_t* e) {
+    cudaError_t rc = cudaEventCreateWithFlags(e, cudaEventDisableTiming);
+    if (rc == cudaSuccess) ev.push_back(*e);
+    return rc;
+  }
+  // `to` waits for everything enqueued on `from` so far
+  cudaError_t order(cudaStream_t from, cudaStream_t to) {
+    cudaEvent_t e;
+    cudaError_t rc = event(&e);
+    if (rc != cudaSuccess) return rc;
+    if ((rc = cudaEventRecord(e, from)) != cudaSuccess) return rc;
+    return cudaStreamWaitEvent(to, e, 0);
+  }
+};
+
+}  // namespace
+
 int idg_grid_host(const idg_plan* plan, const void* vis_host, const void* aterms_host, const float* taper_host,
                   void* grid_host, void* arena_dev, size_t arena_bytes, void* cuda_stream) {
   if (!plan || !vis_host || !aterms_host || !taper_host || !grid_host || !arena_dev) {
@@ -410,18 +494,46 @@ int idg_grid_host(const idg_plan* plan, const void* vis_host, const void* aterms
   char* base = static_cast<char*>(arena_dev);
   const idg_params& p = plan->par;
   const size_t L = p.subgrid_size, Ng = p.grid_size;
-  const size_t vis_b = static_cast<size_t>(plan->n_rows) * p.n_chan * 4 * sizeof(float2);
+  const size_t row_b = static_cast<size_t>(p.n_chan) * 4 * sizeof(float2);
   const size_t at_b = static_cast<size_t>(p.n_stations) * plan->n_intervals * L * L * 4 * sizeof(float2);
   const size_t grid_b = static_cast<size_t>(plan->n_wlayers) * 4 * Ng * Ng * sizeof(float2);
-  IDG_CUDA(cudaMemcpyAsync(base + a.vis, vis_host, vis_b, cudaMemcpyHostToDevice, stream));
-  IDG_CUDA(cudaMemcpyAsync(base + a.aterms, aterms_host, at_b, cudaMemcpyHostToDevice, stream));
-  IDG_CUDA(cudaMemcpyAsync(base + a.taper, taper_host, L * L * sizeof(float), cudaMemcpyHostToDevice, stream));
-  IDG_CUDA(cudaMemcpyAsync(base + a.grid, grid_host, grid_b, cudaMemcpyHostToDevice, stream));
-  int rc = idg_grid(plan, base + a.vis, base + a.aterms, reinterpret_cast<const float*>(base + a.taper), base + a.grid,
-                    base + a.work, a.total - a.work, cuda_stream);
+  const DeviceState* d = nullptr;
+  int rc = ensure_device(plan, &d);
   if (rc != IDG_OK) return rc;
+  ensure_row_runs(plan);
+  // Copy lane: A-terms and taper, then per batch the visibility rows it is the first to read; the grid
+  // (accumulated into) goes up after the first batch's rows, for the first adder.  The compute stream
+  // waits per batch, so uploads overlap the gridding of earlier batches.
+  CopyLane lane;
+  IDG_CUDA(lane.init());
+  IDG_CUDA(lane.order(stream, lane.s));                 // the arena may still be in use by earlier work
+  IDG_CUDA(cudaMemcpyAsync(base + a.aterms, aterms_host, at_b, cudaMemcpyHostToDevice, lane.s));
+  IDG_CUDA(cudaMemcpyAsync(base + a.taper, taper_host, L * L * sizeof(float), cudaMemcpyHostToDevice, lane.s));
+  cudaEvent_t grid_up = nullptr;
+  for (size_t i = 0; i < plan->batches.size(); ++i) {
+    for (const auto& run : plan->rows_first[i])
+      IDG_CUDA(cudaMemcpyAsync(base + a.vis + run.first * row_b, static_cast<const char*>(vis_host) + run.first * row_b,
+                               (run.second - run.first) * row_b, cudaMemcpyHostToDevice, lane.s));
+    IDG_CUDA(lane.order(lane.s, stream));
+    if (i == 0) {
+      IDG_CUDA(cudaMemcpyAsync(base + a.grid, grid_host, grid_b, cudaMemcpyHostToDevice, lane.s));
+      IDG_CUDA(lane.event(&grid_up));
+      IDG_CUDA(cudaEventRecord(grid_up, lane.s));
+    }
+    rc = grid_batch(plan, d, i, base + a.vis, base + a.aterms, reinterpret_cast<const float*>(base + a.taper),
+                    base + a.grid, reinterpret_cast<float2*>(base + a.work), stream, [&]() -> int {
+                      if (i == 0) IDG_CUDA(cudaStreamWaitEvent(stream, grid_up, 0));
+                      return IDG_OK;
+                    });
+    if (rc != IDG_OK) return rc;
+  }
+  if (plan->batches.empty()) {
+    IDG_CUDA(cudaMemcpyAsync(base + a.grid, grid_host, grid_b, cudaMemcpyHostToDevice, lane.s));
+    IDG_CUDA(lane.order(lane.s, stream));
+  }
   IDG_CUDA(cudaMemcpyAsync(grid_host, base + a.grid, grid_b, cudaMemcpyDeviceToHost, stream));
   IDG_CUDA(cudaStreamSynchronize(stream));
+  IDG_CUDA(cudaStreamSynchronize(lane.s));
   return IDG_OK;
 }
 
@@ -437,19 +549,40 @@ int idg_degrid_host(const idg_plan* plan, const void* grid_host, const void* ate
   char* base = static_cast<char*>(arena_dev);
   const idg_params& p = plan->par;
   const size_t L = p.subgrid_size, Ng = p.grid_size;
-  const size_t vis_b = static_cast<size_t>(plan->n_rows) * p.n_chan * 4 * sizeof(float2);
+  const size_t row_b = static_cast<size_t>(p.n_chan) * 4 * sizeof(float2);
+  const size_t vis_b = static_cast<size_t>(plan->n_rows) * row_b;
   const size_t at_b = static_cast<size_t>(p.n_stations) * plan->n_intervals * L * L * 4 * sizeof(float2);
   const size_t grid_b = static_cast<size_t>(plan->n_wlayers) * 4 * Ng * Ng * sizeof(float2);
-  // visibilities not covered by a subgrid must come back untouched: upload them first
-  IDG_CUDA(cudaMemcpyAsync(base + a.vis, vis_host, vis_b, cudaMemcpyHostToDevice, stream));
+  const DeviceState* d = nullptr;
+  int rc = ensure_device(plan, &d);
+  if (rc != IDG_OK) return rc;
+  ensure_row_runs(plan);
+  CopyLane lane;
+  IDG_CUDA(lane.init());
+  IDG_CUDA(lane.order(stream, lane.s));
+  // Visibilities no subgrid covers must come back untouched.  Rows no subgrid touches are simply never
+  // downloaded; rows only partly covered exist only if the planner dropped visibilities, and then the
+  // host's values go up first (on the copy lane, beside the grid upload).
+  const bool partial_rows = plan->n_vis_planned != static_cast<int64_t>(plan->n_rows) * p.n_chan;
+  if (partial_rows) {
+    IDG_CUDA(cudaMemcpyAsync(base + a.vis, vis_host, vis_b, cudaMemcpyHostToDevice, lane.s));
+    IDG_CUDA(lane.order(lane.s, stream));
+  }
+  IDG_CUDA(cudaMemcpyAsync(base + a.grid, grid_host, grid_b, cudaMemcpyHostToDevice, stream));
   IDG_CUDA(cudaMemcpyAsync(base + a.aterms, aterms_host, at_b, cudaMemcpyHostToDevice, stream));
   IDG_CUDA(cudaMemcpyAsync(base + a.taper, taper_host, L * L * sizeof(float), cudaMemcpyHostToDevice, stream));
-  IDG_CUDA(cudaMemcpyAsync(base + a.grid, grid_host, grid_b, cudaMemcpyHostToDevice, stream));
-  int rc = idg_degrid(plan, base + a.grid, base + a.aterms, reinterpret_cast<const float*>(base + a.taper),
-                      base + a.vis, base + a.work, a.total - a.work, cuda_stream);
-  if (rc != IDG_OK) return rc;
-  IDG_CUDA(cudaMemcpyAsync(vis_host, base + a.vis, vis_b, cudaMemcpyDeviceToHost, stream));
+  // per batch: predict, then download the rows it was the last to write while the next batch computes
+  for (size_t i = 0; i < plan->batches.size(); ++i) {
+    rc = degrid_batch(plan, d, i, base + a.grid, base + a.aterms, reinterpret_cast<const float*>(base + a.taper),
+                      base + a.vis, reinterpret_cast<float2*>(base + a.work), stream);
+    if (rc != IDG_OK) return rc;
+    IDG_CUDA(lane.order(stream, lane.s));
+    for (const auto& run : plan->rows_last[i])
+      IDG_CUDA(cudaMemcpyAsync(static_cast<char*>(vis_host) + run.first * row_b, base + a.vis + run.first * row_b,
+                               (run.second - run.first) * row_b, cudaMemcpyDeviceToHost, lane.s));
+  }
   IDG_CUDA(cudaStreamSynchronize(stream));
+  IDG_CUDA(cudaStreamSynchronize(lane.s));
   return IDG_OK;
 }
 

@@ -112,7 +112,9 @@ template <int L, int SIGN>
 __global__ void __launch_bounds__(FftThreads<L>::value) fft_kernel(float2* __restrict__ planes) {
   constexpr int T = FftThreads<L>::value;
   constexpr int R2 = L / 8;
-  constexpr int PITCH = L + 9;                       // row step 1 stores 8 groups of R2 + 1 (conflict-free reads)
+  // Row step 1 stores 8 groups of R2 + 1.  With the pitch = 8 (mod 16) float2, the 4 rows a warp touches in
+  // the row steps land on complementary halves of the 16 8-byte bank slots: every access is conflict-free.
+  constexpr int PITCH = L + 8;
   static_assert(R2 == 4 || R2 == 8 || R2 == 12 || R2 == 16, "L = 8 R2");
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float2* data = reinterpret_cast<float2*>(smem_raw);          // [L][PITCH]
@@ -215,7 +217,7 @@ __global__ void __launch_bounds__(FftThreads<L>::value) fft_kernel(float2* __res
 template <int L>
 cudaError_t launch(int64_t n_planes, float2* planes, int direction, cudaStream_t stream) {
   constexpr int T = FftThreads<L>::value;
-  const size_t smem = static_cast<size_t>(L) * (L + 9) * sizeof(float2) + L * sizeof(float2);
+  const size_t smem = static_cast<size_t>(L) * (L + 8) * sizeof(float2) + L * sizeof(float2);
   if (n_planes == 0) return cudaSuccess;
   cudaError_t e;
   if (direction > 0) {

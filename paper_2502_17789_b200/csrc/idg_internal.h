@@ -4,6 +4,7 @@
 #include <cstdint>
 #include <mutex>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/idg_b200.h"
@@ -70,6 +71,8 @@ struct idg_plan {
   int32_t tiles_x = 0, tiles_y = 0;
   int64_t batch_capacity = 0;             // subgrids per batch
   std::vector<idg::Batch> batches;
+  // rows of the visibility table grouped by the first / last batch that touches them (host-buffer calls)
+  mutable std::vector<std::vector<std::pair<int64_t, int64_t>>> rows_first, rows_last;
   mutable std::mutex mu;
   mutable idg::DeviceState* dev = nullptr;   // uploaded on first device call
 };
