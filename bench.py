@@ -17,6 +17,7 @@ host cores on a bounded sample of the same workload and prints the same line sha
 from __future__ import annotations
 
 import argparse
+import csv
 import json
 import os
 import subprocess
@@ -426,7 +427,8 @@ def run_ours(args):
                                                         sm_obs)
     dom = max(("gridder", "degridder"), key=lambda k: kr[k]["ms_per_step"])
     roofline = {"kernel": dom, "bound": "alu", "achieved": kr[dom]["tflops"], "peak": peak_tflops,
-                "unit": "TFLOP/s", "frac": kr[dom]["frac"], "traffic": None,
+                "unit": "TFLOP/s", "frac": kr[dom]["frac"],
+                "traffic": ncu_traffic(dom, cfg, cnt.n_subgrids, kr[dom]["launches_per_step"]),
                 "peak_basis": f"{N_SM} SM x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {peaks['sm_max_mhz']:.0f} MHz "
                               f"(sm_max_mhz {peaks['source']}); work = 18 FP32-pipe ops per (vis,pixel) pair",
                 "frac_at_observed_clock": kr[dom]["frac_at_observed_clock"],
@@ -442,6 +444,20 @@ def run_ours(args):
     if world > 1:
         dist.destroy_process_group()
     return 0
+
+
+def ncu_traffic(kernel, cfg, n_subgrids, launches_per_step):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/), scaled from the
+    captured launch to this run's average launch; None when there is no capture for this workload."""
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "dram_traffic_r01f.csv")
+    if cfg.config_id != 2 or not os.path.exists(path) or not launches_per_step:
+        return None
+    with open(path) as f:
+        for row in csv.DictReader(f):
+            if row["kernel"] == kernel:
+                per_subgrid = (float(row["dram_bytes_read"]) + float(row["dram_bytes_write"])) / float(row["subgrids_in_launch"])
+                return per_subgrid * n_subgrids / launches_per_step
+    return None
 
 
 def main():

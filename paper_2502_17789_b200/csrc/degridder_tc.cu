@@ -293,6 +293,9 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, 1)
 #pragma unroll
         for (int s = 0; s < NA; ++s) {
           const bool valid = left > 0;
+          // the previous slot goes to the service warp before this one's arithmetic
+          if (s > 0) hand_off(gbar + 8 * (s - 1));
+          else if (pending) hand_off(gbar + 8 * (NA - 1));
           uint32_t hi[16], lo[16];
           if (valid) {
             if (cl == 0) {
@@ -333,9 +336,6 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, 1)
               lo[4 * j2 + 3] = __float_as_uint(l1.y);
             }
           }
-          // the previous slot: its stores finished long ago
-          if (s > 0) hand_off(gbar + 8 * (s - 1));
-          else if (pending) hand_off(gbar + 8 * (NA - 1));
           if (need_wait) tc::mbar_wait(gbar + 8 * NA + 8 * s, phase ^ 1);            // MMAs of the last revolution
           if (valid) {
             tc::tmem_st16(gtmem + s * A_COLS, hi);

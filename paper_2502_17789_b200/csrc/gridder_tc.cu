@@ -328,6 +328,10 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, 1)
 #pragma unroll
           for (int s = 0; s < NA; ++s) {
             const bool valid = left > 0;
+            // the previous slot goes to the service warp before this one's arithmetic: its stores were
+            // issued a whole hand-off / wait / store sequence ago
+            if (s > 0) hand_off(gbar + 8 * (s - 1));
+            else if (pending) hand_off(gbar + 8 * (NA - 1));
             uint32_t hi[KC / 8][16], lo[KC / 8][16];
             if (valid) {
 #pragma unroll
@@ -358,9 +362,6 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, 1)
                 }
               }
             }
-            // the previous slot: its stores finished long ago
-            if (s > 0) hand_off(gbar + 8 * (s - 1));
-            else if (pending) hand_off(gbar + 8 * (NA - 1));
             if (need_wait) tc::mbar_wait(gbar + 8 * NA + 8 * s, phase ^ 1);          // MMAs of the last revolution
             if (valid) {
 #pragma unroll
