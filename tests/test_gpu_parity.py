@@ -293,3 +293,88 @@ def test_empty_and_error_paths(idg):
     ws = torch.empty(plan.workspace_bytes(), dtype=torch.uint8, device=DEV)
     idg.grid(plan, d_vis, d_at, d_tp, d_grid, ws)
     assert idg.launch_count() == before + 3                          # gridder, fft, adder
+
+
+@pytest.mark.parametrize("variant", ["simt", "tensor"])
+def test_full_path_config2_shape(idg, variant):
+    """The whole path on a config-2-shaped observation (64 x 64 subgrids, 32 channels, 256 visibilities per
+    subgrid) small enough for the oracle to grid in full, with each pair of direct-sum kernels."""
+    request_variant(idg, variant, kind="gridder")
+    request_variant(idg, variant, kind="degridder")
+    cfg = synth.scaled(synth.get_config(2), n_stations=8, n_times=16, grid_size=1024, cell_arcsec=120.0)
+    obs, par, plan, sub = setup(idg, cfg, vis="hash", max_batch_subgrids=11)
+    cnt = plan.counts()
+    Ng = cfg.grid_size
+    d_vis, d_at, d_tp = dev(obs.vis), dev(obs.aterms), dev(obs.taper)
+    d_grid = torch.zeros((cnt.n_wlayers, 4, Ng, Ng), dtype=torch.complex64, device=DEV)
+    ws = torch.empty(plan.workspace_bytes(), dtype=torch.uint8, device=DEV)
+    idg.grid(plan, d_vis, d_at, d_tp, d_grid, ws)
+    ref = orc.grid(par, sub, obs.uvw, obs.freqs, obs.vis, obs.baselines, obs.aterms, obs.taper)
+    assert nerr(d_grid.cpu().numpy(), ref) <= TOL
+    d_grid2 = torch.zeros_like(d_grid)
+    idg.grid(plan, d_vis, d_at, d_tp, d_grid2, ws)
+    assert torch.equal(torch.view_as_real(d_grid), torch.view_as_real(d_grid2)), "not bitwise reproducible"
+    G = ref.astype(np.complex64)
+    d_out = torch.zeros((cfg.n_rows, cfg.n_chan, 4), dtype=torch.complex64, device=DEV)
+    idg.degrid(plan, dev(G), d_at, d_tp, d_out, ws)
+    vref = orc.degrid(par, sub, obs.uvw, obs.freqs, G, obs.baselines, obs.aterms, obs.taper)
+    assert nerr(d_out.cpu().numpy(), vref) <= TOL
+
+
+def test_full_size_config2_sampled(idg):
+    """BASELINE.json configs[1] at full size, in the launch configuration bench.py times (default plan, AUTO
+    kernels = tensor-core), checked on outputs the oracle computes one by one:
+      * master-grid pixels in sparsely covered tiles: the oracle grids every subgrid overlapping the pixel;
+      * predicted visibilities of sampled subgrids, from the same master grid through splitter, inverse FFT,
+        A-terms / taper and the degridder of the oracle;
+      * every planned visibility written, run-to-run bitwise identical grids."""
+    cfg = synth.get_config(2)
+    obs = synth.make_observation(cfg, vis="hash")
+    par = oracle_params(cfg)
+    plan = idg.plan_from_config(cfg, obs.uvw, obs.freqs, obs.baselines)
+    sub = plan.export()
+    cnt = plan.counts()
+    assert cnt.n_subgrids == 56896 and cnt.n_vis_dropped == 0
+    L, Ng = cfg.subgrid_size, cfg.grid_size
+    d_vis, d_at, d_tp = dev(obs.vis), dev(obs.aterms), dev(obs.taper)
+    d_grid = torch.zeros((cnt.n_wlayers, 4, Ng, Ng), dtype=torch.complex64, device=DEV)
+    ws = torch.empty(plan.workspace_bytes(), dtype=torch.uint8, device=DEV)
+    idg.grid(plan, d_vis, d_at, d_tp, d_grid, ws)
+    d_grid2 = torch.zeros_like(d_grid)
+    idg.grid(plan, d_vis, d_at, d_tp, d_grid2, ws)
+    assert torch.equal(torch.view_as_real(d_grid), torch.view_as_real(d_grid2)), "not bitwise reproducible"
+    del d_grid2
+    g = d_grid.cpu().numpy()
+
+    # --- grid pixels covered by few subgrids (the outskirts of the uv coverage)
+    x0, y0 = sub[:, 5].astype(np.int64), sub[:, 6].astype(np.int64)
+    rng = np.random.default_rng(11)
+    scale = float(np.abs(g).max())
+    cands = []
+    for s in rng.choice(len(sub), 3000, replace=False):
+        py, px = int(y0[s] + rng.integers(L)), int(x0[s] + rng.integers(L))
+        cover = np.nonzero((x0 <= px) & (px < x0 + L) & (y0 <= py) & (py < y0 + L))[0]
+        cands.append((len(cover), py, px, cover))
+    cands.sort(key=lambda c: c[0])
+    picks = cands[:4] + cands[len(cands) // 8: len(cands) // 8 + 2]     # the sparsest and two busier pixels
+    assert picks[-1][0] <= 400, "sampled pixels are too expensive for the oracle"
+    for _, py, px, cover in picks:
+        want = np.zeros(4, np.complex128)
+        for c in cover:
+            _, Shat = orc.grid_subgrid(par, sub[c], obs.uvw, obs.freqs, obs.vis, obs.baselines, obs.aterms, obs.taper)
+            want += Shat[py - y0[c], px - x0[c], :]
+        got = g[0, :, py, px]
+        assert np.abs(got - want).max() <= TOL * max(scale, np.abs(want).max()), (py, px, cover.tolist(), got, want)
+
+    # --- prediction of sampled subgrids from this grid
+    d_out = torch.full((cfg.n_rows, cfg.n_chan, 4), float("nan"), dtype=torch.complex64, device=DEV)
+    idg.degrid(plan, d_grid, d_at, d_tp, d_out, ws)
+    out = d_out.cpu().numpy()
+    assert not np.isnan(out.view(np.float32)).any(), "a planned visibility was not written"
+    for s in sample_subgrids(sub, 6, seed=3):
+        b, t0, nt, c0, nc = (int(v) for v in sub[s][:5])
+        _, ref = orc.degrid_subgrid(par, sub[s], obs.uvw, obs.freqs, g, cnt.wl_min, obs.baselines, obs.aterms,
+                                    obs.taper)
+        r0 = b * cfg.n_times + t0
+        e = nerr(out[r0:r0 + nt, c0:c0 + nc], ref)
+        assert e <= TOL, (s, sub[s].tolist(), e)
