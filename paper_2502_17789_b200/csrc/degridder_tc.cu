@@ -35,7 +35,7 @@ namespace idg {
 namespace {
 
 #ifndef IDG_DTC_NG
-#define IDG_DTC_NG 4
+#define IDG_DTC_NG 2
 #endif
 #ifndef IDG_DTC_DG
 #define IDG_DTC_DG 6
@@ -65,9 +65,9 @@ __device__ __forceinline__ float dtc_round(float x) {
 }
 
 template <int L, int NG, int DG, int NA, int NS>
-__global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, 1)
+__global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 2 ? 2 : 1)
     degridder_tc_kernel(const SubgridJob job, const float2* __restrict__ in, float4* __restrict__ vis) {
-  static_assert((L * L) % kStagePix == 0 && L % kKC == 0 && NG == 4 && (NS & (NS - 1)) == 0, "shape");
+  static_assert((L * L) % kStagePix == 0 && L % kKC == 0 && (NG == 2 || NG == 4) && (NS & (NS - 1)) == 0, "shape");
   static_assert(DG % NA == 0, "an accumulator group is a whole number of ring revolutions");
   constexpr int NSTAGES = (L * L) / kStagePix;
   constexpr int A_COLS = 4 * kKC;                      // per slot: heads [0, 16), remainders [16, 32)
@@ -135,7 +135,7 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, 1)
 
   for (int t_base = 0; t_base < T; t_base += NG, sc0 += NSTAGES) {
     const int t_round = min(NG, T - t_base);           // tiles of this round
-    const int lgP = t_round == 1 ? 2 : (t_round == 2 ? 1 : 0);   // groups per tile P = 1 << lgP
+    const int lgP = t_round == 1 ? (NG == 4 ? 2 : 1) : ((t_round == 2 && NG == 4) ? 1 : 0);   // groups per tile P = 1 << lgP
     const int tile_l = gi % t_round, part = gi / t_round;
     const bool active = part < (1 << lgP);
     const int lgn = 5 - lgP;                           // a part's chunks per stage: ncs = 1 << lgn
@@ -385,10 +385,13 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, 1)
   if (warp == NG * 4) tc::tmem_dealloc(tmem, TMEM_COLS);
 }
 
+// Two groups per CTA with a two-stage B ring let two CTAs (different subgrids) share an SM, so one CTA's
+// prologue and end-of-round reduction overlap the other's arithmetic; four groups and four stages make one
+// CTA per SM.  IDG_DTC_NG picks; the default is the measured winner on config 2.
 template <int L>
 cudaError_t launch(const SubgridJob& job, const float2* in, float4* vis, cudaStream_t stream) {
   if (job.count == 0) return cudaSuccess;
-  constexpr int NG = IDG_DTC_NG, NS = IDG_DTC_NS;
+  constexpr int NG = IDG_DTC_NG, NS = NG == 2 ? 2 : IDG_DTC_NS;
   constexpr size_t dyn = NS * kStageBBytes + NS * kStagePix * 4 + (NG - 1) * kTileV * 8 * 4;
   auto kernel = degridder_tc_kernel<L, NG, IDG_DTC_DG, IDG_DTC_NA, NS>;
   static bool configured = false;                      // per instantiation

@@ -19,7 +19,8 @@
 // (round-to-nearest adds) every DG chunks, alternating two TMEM accumulators so that draining one
 // overlaps the MMAs into the other.
 //
-// One CTA per subgrid: NG groups of 128 compute threads plus one service warp.
+// One CTA per subgrid: NG groups of 128 compute threads plus one service warp per group; NG = 1, 2 or 4
+// chosen at launch so that 4 / NG CTAs share an SM (see launch_l).
 //   all threads      stage the B operand of the subgrid's visibilities ONCE in shared memory (heads
 //                    and remainders, canonical K-major core-matrix layout); every pixel tile reuses it.
 //                    Subgrids with more visibilities than fit are processed in segments of whole table
@@ -46,9 +47,6 @@ namespace {
 
 #ifndef IDG_TC_KC
 #define IDG_TC_KC 8
-#endif
-#ifndef IDG_TC_NG
-#define IDG_TC_NG 4
 #endif
 #ifndef IDG_TC_DG
 #define IDG_TC_DG 6
@@ -77,7 +75,7 @@ __device__ __forceinline__ float tf32_round(float x) {
 // NG = compute groups (tiles in flight) per CTA, KC = visibilities per chunk, DG = chunks per accumulator
 // group, NA = depth of a group's A ring in TMEM
 template <int L, int NG, int KC, int DG, int NA>
-__global__ void __launch_bounds__(NG* kTileM + NG * 32, 1)
+__global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ? 2 : 1))
     gridder_tc_kernel(const SubgridJob job, const float4* __restrict__ vis, float2* __restrict__ out,
                       const int cap_chunks) {
   constexpr int TILES = (L * L) / kTileM;
@@ -430,13 +428,23 @@ cudaError_t launch(const SubgridJob& job, const float4* vis, float2* out, cudaSt
   return cudaGetLastError();
 }
 
-// largest group count <= want that divides the subgrid's tile count
-constexpr int groups_per_cta(int L, int want) {
-  const int tiles = L * L / kTileM;
-  int g = 1;
-  for (int d = 1; d <= want && d <= tiles; ++d)
-    if (tiles % d == 0) g = d;
-  return g;
+// Groups per CTA.  Tensor memory holds four groups per SM whatever the split; with fewer groups per CTA
+// several CTAs (different subgrids) share the SM, so one CTA's prologue (B staging, row constants) and
+// tail overlap the others' arithmetic: measured 4.73 (1 group x 4 CTAs), 4.65 (2 x 2), 4.53 (4 x 1)
+// pairs/clk/SM on config 2.  What decides is whether the CTAs' B operands fit shared memory side by side.
+template <int L>
+cudaError_t launch_l(const SubgridJob& job, const float4* vis, float2* out, cudaStream_t stream) {
+  constexpr int KC = IDG_TC_KC;
+  const size_t dyn = static_cast<size_t>(std::min(job.max_nt * ((job.n_chan + KC - 1) / KC), kMaxBBytes / (KC * 128))) *
+                     (KC * 128);
+  constexpr size_t kStaticAndReserved = 11 * 1024, kSmemPerSm = 227 * 1024;
+#ifdef IDG_TC_NG
+  return launch<L, IDG_TC_NG, KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
+#else
+  if (4 * (dyn + kStaticAndReserved) <= kSmemPerSm) return launch<L, 1, KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
+  if (2 * (dyn + kStaticAndReserved) <= kSmemPerSm) return launch<L, 2, KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
+  return launch<L, 4, KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
+#endif
 }
 
 }  // namespace
@@ -448,10 +456,10 @@ cudaError_t launch_gridder_tc(const SubgridJob& job, const float4* vis, float2* 
       (job.n_chan + KC - 1) / KC > kMaxBBytes / (KC * 128))
     return launch_gridder(job, vis, out, stream);
   switch (job.subgrid_size) {
-    case 32:  return launch<32, groups_per_cta(32, IDG_TC_NG), KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
-    case 64:  return launch<64, groups_per_cta(64, IDG_TC_NG), KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
-    case 96:  return launch<96, groups_per_cta(96, IDG_TC_NG), KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
-    case 128: return launch<128, groups_per_cta(128, IDG_TC_NG), KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
+    case 32:  return launch_l<32>(job, vis, out, stream);
+    case 64:  return launch_l<64>(job, vis, out, stream);
+    case 96:  return launch_l<96>(job, vis, out, stream);
+    case 128: return launch_l<128>(job, vis, out, stream);
     default:  return cudaErrorInvalidValue;
   }
 }
