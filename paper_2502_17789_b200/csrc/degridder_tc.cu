@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
   const uint32_t gtmem = tc::opaque(tmem + gi * GCOLS + (static_cast<uint32_t>((warp & 3) * 32) << 16));
   const int tpix = tid & (kTileV - 1);
 
-  int q = 0, revs = 0;                                 // accumulator groups closed, ring revolutions done
+  int q = 0;                                           // accumulator groups closed
   uint32_t phase = 0;                                  // parity of the current revolution
   int sc0 = 0;                                         // stages streamed before this round
 
@@ -206,7 +206,7 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
         for (int rev = 0; rev < nrev; ++rev) {
           const bool group_last = rig == RPG - 1 || rev == nrev - 1;
           const uint32_t d0 = gt + D_COL + 16 * (q & 1);
-          if (rig == 0 && q >= 2)                      // accumulator q & 1 drained (group q - 2)
+          if (rig == 0)                                // accumulator q & 1 drained (group q - 2; fresh barriers pass)
             tc::mbar_wait(sbar + 16 * NA + 16 + 8 * (q & 1), ((q - 2) >> 1) & 1);
 #pragma unroll
           for (int s = 0; s < NA; ++s) {
@@ -289,7 +289,6 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
       const int lp0 = static_cast<int>(tc::opaque(static_cast<uint32_t>((part << lgn) * kKC)));
       int left = total, cl = 0, st = 0, rig = 0, gin = 0;
       for (int rev = 0; rev < nrev; ++rev) {
-        const bool need_wait = revs > 0;               // slots were used before: wait for their MMAs
 #pragma unroll
         for (int s = 0; s < NA; ++s) {
           const bool valid = left > 0;
@@ -336,7 +335,7 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
               lo[4 * j2 + 3] = __float_as_uint(l1.y);
             }
           }
-          if (need_wait) tc::mbar_wait(gbar + 8 * NA + 8 * s, phase ^ 1);            // MMAs of the last revolution
+          tc::mbar_wait(gbar + 8 * NA + 8 * s, phase ^ 1);            // MMAs of the last revolution (a fresh barrier passes parity 1)
           if (valid) {
             tc::tmem_st16(gtmem + s * A_COLS, hi);
             tc::tmem_st16(gtmem + s * A_COLS + 2 * kKC, lo);
@@ -349,7 +348,6 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
         }
         pending = true;
         phase ^= 1;
-        ++revs;
         if (++rig == RPG || rev == nrev - 1) {
           // group q closes; group q - 1 was handed over a group ago, so its MMAs are done
           if (gin > 0) drain(q - 1);

@@ -173,7 +173,7 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
   // dempty[p] at + 16 NA + 16.  `opaque` keeps them in registers.
   const uint32_t gbar = tc::opaque(bar0 + 8 * mygroup * NBAR);
   const uint32_t gtmem = tc::opaque(tmem + mygroup * GCOLS + (static_cast<uint32_t>((warp & 3) * 32) << 16));
-  int q = 0, revs = 0;                                 // accumulator groups closed, ring revolutions done
+  int q = 0;                                           // accumulator groups closed
   uint32_t phase = 0;                                  // parity of the current revolution
 
   const int tpix = tid & (kTileM - 1);
@@ -229,7 +229,7 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
         for (int rev = 0; rev < nrev_u; ++rev) {
           const bool group_last = rig == RPG - 1 || rev == nrev_u - 1;
           const uint32_t d0 = gt + D_COL + 16 * (q & 1);
-          if (rig == 0 && q >= 2)                      // accumulator q & 1 drained (group q - 2)
+          if (rig == 0)                                // accumulator q & 1 drained (group q - 2; fresh barriers pass)
             tc::mbar_wait(sbar + 16 * NA + 16 + 8 * (q & 1), ((q - 2) >> 1) & 1);
 #pragma unroll
           for (int s = 0; s < NA; ++s) {
@@ -322,7 +322,6 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
         int rig = 0, gin = 0;                          // revolutions in the current group, groups closed in this tile
         int left = nchunks;                            // chunks of this tile still to store
         for (int rev = 0; rev < nrev; ++rev) {
-          const bool need_wait = revs > 0;             // slots were used before: wait for their MMAs
 #pragma unroll
           for (int s = 0; s < NA; ++s) {
             const bool valid = left > 0;
@@ -360,7 +359,7 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
                 }
               }
             }
-            if (need_wait) tc::mbar_wait(gbar + 8 * NA + 8 * s, phase ^ 1);          // MMAs of the last revolution
+            tc::mbar_wait(gbar + 8 * NA + 8 * s, phase ^ 1);          // MMAs of the last revolution (a fresh barrier passes parity 1)
             if (valid) {
 #pragma unroll
               for (int half = 0; half < KC / 8; ++half) {
@@ -379,7 +378,6 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
           }
           pending = true;
           phase ^= 1;
-          ++revs;
           if (++rig == RPG || rev == nrev - 1) {
             // group q closes; group q - 1 was handed over a group ago, so its MMAs are done
             if (ppix >= 0) {
