@@ -347,10 +347,9 @@ int degrid_batch(const idg_plan* plan, const DeviceState* d, size_t i, const voi
   const int L = plan->par.subgrid_size, Ng = plan->par.grid_size;
   const Batch& bt = plan->batches[i];
   const SubgridJob job = make_job(plan, d, bt.first, bt.count, aterms_dev, taper_dev);
-  { ProfScope ps(IDG_K_SPLITTER, stream);
-    IDG_CUDA(launch_splitter(d->meta, bt.first, bt.count, L, Ng, static_cast<const float2*>(grid_dev), stack, stream)); }
+  // splitter (a6) and inverse subgrid FFT (a7) in one kernel: the transform gathers its input from the grid
   { ProfScope ps(IDG_K_IFFT, stream);
-    IDG_CUDA(launch_subgrid_fft(L, bt.count * 4, stack, -1, stream)); }
+    IDG_CUDA(launch_split_ifft(d->meta, bt.first, bt.count, L, Ng, static_cast<const float2*>(grid_dev), stack, stream)); }
   { ProfScope ps(IDG_K_DEGRIDDER, stream);
     IDG_CUDA(run_degridder(plan, job, stack, static_cast<float4*>(vis_dev), stream)); }
   return IDG_OK;

@@ -38,7 +38,7 @@ namespace {
 #define IDG_DTC_NG 2
 #endif
 #ifndef IDG_DTC_DG
-#define IDG_DTC_DG 6
+#define IDG_DTC_DG 12
 #endif
 #ifndef IDG_DTC_NA
 #define IDG_DTC_NA 3

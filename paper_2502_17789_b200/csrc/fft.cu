@@ -108,8 +108,16 @@ __device__ __forceinline__ void dft_small(float2 (&x)[N]) {
 template <int L>
 struct FftThreads { static constexpr int value = L == 32 ? 128 : (L == 64 ? 256 : (L == 96 ? 576 : 512)); };
 
+// Where the transform reads its input: the plane itself (in place), or, for the prediction direction, the
+// master grid patch under the subgrid (step a6, the splitter, fused into the load of step a7).
+struct GridSource {
+  const float2* grid;      // [W, 4, Ng, Ng]; nullptr = in place
+  const int32_t* meta;     // subgrid metadata of plane 0's subgrid onwards
+  int Ng;
+};
+
 template <int L, int SIGN>
-__global__ void __launch_bounds__(FftThreads<L>::value) fft_kernel(float2* __restrict__ planes) {
+__global__ void __launch_bounds__(FftThreads<L>::value) fft_kernel(float2* __restrict__ planes, const GridSource src) {
   constexpr int T = FftThreads<L>::value;
   constexpr int R2 = L / 8;
   // Row step 1 stores 8 groups of R2 + 1.  With the pitch = 8 (mod 16) float2, the 4 rows a warp touches in
@@ -121,6 +129,15 @@ __global__ void __launch_bounds__(FftThreads<L>::value) fft_kernel(float2* __res
   float2* tw = data + L * PITCH;                               // [L] exp(SIGN 2 pi i m / L)
   float2* plane = planes + static_cast<int64_t>(blockIdx.x) * L * L;
   const int tid = threadIdx.x;
+  // input rows: `in` + r * in_pitch
+  const float2* in = plane;
+  int64_t in_pitch = L;
+  if (src.grid != nullptr) {
+    const int32_t* m = src.meta + static_cast<int64_t>(blockIdx.x >> 2) * kMetaStride;
+    const int x0 = m[5], y0 = m[6], layer = m[11], pol = blockIdx.x & 3;
+    in = src.grid + ((static_cast<int64_t>(layer) * 4 + pol) * src.Ng + y0) * src.Ng + x0;
+    in_pitch = src.Ng;
+  }
 
   for (int k = tid; k < L; k += T) {
     float s, c;
@@ -139,7 +156,7 @@ __global__ void __launch_bounds__(FftThreads<L>::value) fft_kernel(float2* __res
       const float sg = ((r + n2) & 1) ? -1.f : 1.f;   // checkerboard; R2 is even, so n1 R2 drops out
 #pragma unroll
       for (int n1 = 0; n1 < 8; ++n1) {
-        const float2 v = plane[r * L + n1 * R2 + n2];
+        const float2 v = in[r * in_pitch + n1 * R2 + n2];
         xr[it][n1] = make_float2(v.x * sg, v.y * sg);
       }
       dft_small<8, SIGN>(xr[it]);
@@ -215,7 +232,7 @@ __global__ void __launch_bounds__(FftThreads<L>::value) fft_kernel(float2* __res
 }
 
 template <int L>
-cudaError_t launch(int64_t n_planes, float2* planes, int direction, cudaStream_t stream) {
+cudaError_t launch(int64_t n_planes, float2* planes, int direction, const GridSource& src, cudaStream_t stream) {
   constexpr int T = FftThreads<L>::value;
   const size_t smem = static_cast<size_t>(L) * (L + 8) * sizeof(float2) + L * sizeof(float2);
   if (n_planes == 0) return cudaSuccess;
@@ -223,11 +240,11 @@ cudaError_t launch(int64_t n_planes, float2* planes, int direction, cudaStream_t
   if (direction > 0) {
     e = cudaFuncSetAttribute(fft_kernel<L, -1>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
     if (e != cudaSuccess) return e;
-    fft_kernel<L, -1><<<static_cast<unsigned>(n_planes), T, smem, stream>>>(planes);
+    fft_kernel<L, -1><<<static_cast<unsigned>(n_planes), T, smem, stream>>>(planes, src);
   } else {
     e = cudaFuncSetAttribute(fft_kernel<L, +1>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
     if (e != cudaSuccess) return e;
-    fft_kernel<L, +1><<<static_cast<unsigned>(n_planes), T, smem, stream>>>(planes);
+    fft_kernel<L, +1><<<static_cast<unsigned>(n_planes), T, smem, stream>>>(planes, src);
   }
   count_launch();
   return cudaGetLastError();
@@ -236,11 +253,24 @@ cudaError_t launch(int64_t n_planes, float2* planes, int direction, cudaStream_t
 }  // namespace
 
 cudaError_t launch_subgrid_fft(int L, int64_t n_planes, float2* planes, int direction, cudaStream_t stream) {
+  const GridSource none{nullptr, nullptr, 0};
   switch (L) {
-    case 32:  return launch<32>(n_planes, planes, direction, stream);
-    case 64:  return launch<64>(n_planes, planes, direction, stream);
-    case 96:  return launch<96>(n_planes, planes, direction, stream);
-    case 128: return launch<128>(n_planes, planes, direction, stream);
+    case 32:  return launch<32>(n_planes, planes, direction, none, stream);
+    case 64:  return launch<64>(n_planes, planes, direction, none, stream);
+    case 96:  return launch<96>(n_planes, planes, direction, none, stream);
+    case 128: return launch<128>(n_planes, planes, direction, none, stream);
+    default:  return cudaErrorInvalidValue;
+  }
+}
+
+cudaError_t launch_split_ifft(const int32_t* meta, int64_t first, int64_t count, int L, int Ng, const float2* grid,
+                              float2* subgrids, cudaStream_t stream) {
+  const GridSource src{grid, meta + first * kMetaStride, Ng};
+  switch (L) {
+    case 32:  return launch<32>(count * 4, subgrids, -1, src, stream);
+    case 64:  return launch<64>(count * 4, subgrids, -1, src, stream);
+    case 96:  return launch<96>(count * 4, subgrids, -1, src, stream);
+    case 128: return launch<128>(count * 4, subgrids, -1, src, stream);
     default:  return cudaErrorInvalidValue;
   }
 }

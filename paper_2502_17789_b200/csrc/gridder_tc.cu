@@ -49,7 +49,7 @@ namespace {
 #define IDG_TC_KC 8
 #endif
 #ifndef IDG_TC_DG
-#define IDG_TC_DG 6
+#define IDG_TC_DG 12
 #endif
 #ifndef IDG_TC_NA
 #define IDG_TC_NA 3

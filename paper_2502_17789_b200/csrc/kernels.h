@@ -42,6 +42,11 @@ cudaError_t launch_degridder_tc(const SubgridJob& job, const float2* in, float4*
 // steps a4 / a7: centred L x L DFT of n_planes planes in place, scaled by 1/L^2.
 cudaError_t launch_subgrid_fft(int L, int64_t n_planes, float2* planes, int direction, cudaStream_t stream);
 
+// steps a6 + a7 in one pass: the inverse transform reads the master grid patch under each subgrid
+// (the splitter's gather) instead of the stack, and writes the image-domain subgrid to the stack.
+cudaError_t launch_split_ifft(const int32_t* meta, int64_t first, int64_t count, int L, int Ng, const float2* grid,
+                              float2* subgrids, cudaStream_t stream);
+
 // step a5: tile-owner adder.  csr lists, per non-empty tile, the subgrids overlapping it.
 cudaError_t launch_adder(const int32_t* meta, const DeviceCsr& csr, int64_t first, int L, int Ng,
                          int tiles_x, int tiles_y, const float2* subgrids, float2* grid,
