@@ -151,7 +151,7 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
       const int pw = uwarp - NG * 5;                   // producer warp index
       for (int st = 0; st < NSTAGES; ++st) {
         const int gst = sc0 + st, slot = gst & (NS - 1);
-        if (gst >= NS) tc::mbar_wait(bar_sempty + 8 * slot, ((gst / NS) - 1) & 1);
+        if (gst >= NS) tc::mbar_wait_backoff(bar_sempty + 8 * slot, ((gst / NS) - 1) & 1, 256);
         float* Bs = reinterpret_cast<float*>(sB + slot * kStageBBytes);
 #ifdef IDG_DTC_FAKE_PRODUCER
         if (gst < NS)
