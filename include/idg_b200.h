@@ -22,8 +22,11 @@
  *   2x2 matrices are row-major: vis[r, c, 0..3] = (XX, XY, YX, YY); Jones M[st, it, y, x, 2, 2].
  *
  * All *_dev pointers are caller-owned device memory (16-byte aligned); all *_host pointers are
- * caller-owned host memory.  The library allocates on the device only the plan metadata it
- * uploads on first use (freed by idg_plan_destroy).  All device work is enqueued on the
+ * caller-owned host memory.  The library allocates on the device only what belongs to the plan:
+ * the metadata it uploads on first use and the adder's scratch (fp64 partial sums of the tile
+ * segments, one counter per tile), both freed by idg_plan_destroy.  Because that scratch is per
+ * plan, calls on ONE plan must not overlap in time (one stream at a time); different plans are
+ * independent.  All device work is enqueued on the
  * caller's stream (a cudaStream_t passed as void*; NULL = default stream) and the calls return
  * without synchronising unless stated.  Every function returns 0 on success or a negative
  * IDG_E* code; idg_last_error() gives a thread-local message.  There is no CPU fallback: a
@@ -116,10 +119,14 @@ IDG_API int  idg_grid(const idg_plan* plan, const void* vis_dev, const void* ate
 IDG_API int  idg_degrid(const idg_plan* plan, const void* grid_dev, const void* aterms_dev, const float* taper_dev,
                 void* vis_dev, void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
 
-/* ---- the same two calls on HOST buffers (pinned memory recommended).  They copy the inputs
- * to `arena_dev`, run the device path on `cuda_stream`, copy the result back (grid_host is
- * accumulated into: it is uploaded first) and synchronise the stream before returning.
- * arena_dev must hold idg_host_arena_bytes(plan, direction) bytes. */
+/* ---- the same two calls on HOST buffers (pinned memory recommended: pageable memory makes the
+ * copies synchronous).  They copy the inputs to `arena_dev`, run the device path on `cuda_stream`,
+ * copy the result back (grid_host is accumulated into: it is uploaded too) and synchronise before
+ * returning.  Copies run on a second stream and overlap compute batch by batch: a visibility row
+ * goes up just before the first batch that reads it and comes down right after the last batch
+ * that writes it, so a plan with smaller batches (idg_params.max_batch_subgrids) overlaps more.
+ * idg_degrid_host uploads vis_host only when the planner left visibilities uncovered (they come
+ * back untouched).  arena_dev must hold idg_host_arena_bytes(plan, direction) bytes. */
 IDG_API size_t idg_host_arena_bytes(const idg_plan* plan, int direction);
 IDG_API int  idg_grid_host(const idg_plan* plan, const void* vis_host, const void* aterms_host,
                    const float* taper_host, void* grid_host, void* arena_dev, size_t arena_bytes,
