@@ -41,6 +41,22 @@ FP32_OPS_PER_PAIR = 18           # 16 FFMA (2x2 complex MAC) + 1 phase FFMA + 1 
 MUFU_PER_PAIR = 2
 
 
+def replicas_aggregate(local_seconds, units_per_rank, world, group=None):
+    """Whole-job figures of N independent replicas (the path does not shard in this
+    build, so every rank runs the same workload with no data-path collective).  The job's time is the MAX
+    over ranks of the device-timed region, and the job processed world x units_per_rank units in it.
+    Returns (seconds, units per second).  Works on any backend (the CPU tests run it over gloo)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(local_seconds)], dtype=torch.float64)
+    if world > 1:
+        if dist.get_backend(group) == "nccl":
+            t = t.cuda()
+        dist.all_reduce(t, op=dist.ReduceOp.MAX, group=group)
+    seconds = float(t.item())
+    return seconds, world * units_per_rank / seconds
+
+
 def load_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -366,12 +382,10 @@ def run_ours(args):
     total_ms = ev[0].elapsed_time(ev[-1])
     grid_ms = sum(ev[2 * k].elapsed_time(ev[2 * k + 1]) for k in range(args.steps)) / args.steps
     degrid_ms = sum(ev[2 * k + 1].elapsed_time(ev[2 * k + 2]) for k in range(args.steps)) / args.steps
-    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
-    ms_per_step = total_ms / args.steps
     n_vis = cnt.n_vis_planned
+    total_s, value = replicas_aggregate(total_ms / 1e3, n_vis * args.steps, world)
+    total_ms = total_s * 1e3
+    ms_per_step = total_ms / args.steps
 
     # end to end through the host-buffer C-ABI calls: pinned host -> device -> pinned host, every step
     e2e = None
@@ -399,10 +413,7 @@ def run_ours(args):
             idg.degrid_host(plan, h_grid, h_at, h_tp, h_out, arena, stream)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        te = torch.tensor([dt], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        dt = float(te.item())
+        dt, e2e_value = replicas_aggregate(dt, n_vis * n_e2e, world)
         nb = lambda x: x.numel() * x.element_size()  # noqa: E731
         # grid call: visibilities, A-terms, taper, grid up; degrid call: grid, A-terms, taper up, and the
         # visibilities only when the planner left some uncovered (they must come back untouched)
@@ -410,7 +421,7 @@ def run_ours(args):
         h2d = (nb(h_vis) + nb(h_at) + nb(h_tp) + nb(h_grid)) + (nb(h_at) + nb(h_tp) + nb(h_grid)) \
             + (0 if covered else nb(h_vis))
         d2h = nb(h_grid) + nb(h_out)
-        e2e = {"value": world * n_vis * n_e2e / dt, "unit": UNIT, "h2d_bytes_per_step": h2d,
+        e2e = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "steps": n_e2e, "ms_per_step": 1e3 * dt / n_e2e,
                "api": "idg_grid_host + idg_degrid_host (pinned host buffers; copies inside the calls, "
                       "overlapped with compute per batch on a second stream)",
@@ -433,7 +444,7 @@ def run_ours(args):
                               f"(sm_max_mhz {peaks['source']}); work = 18 FP32-pipe ops per (vis,pixel) pair",
                 "frac_at_observed_clock": kr[dom]["frac_at_observed_clock"],
                 "hbm_frac_of_measured": kr[dom]["hbm_frac"], "hbm_peak_gbs": peaks["hbm_gbs"]}
-    line = {"metric": METRIC, "value": world * n_vis / (ms_per_step / 1e3), "unit": UNIT, "n_gpus": world,
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": workload_config(cfg), "grid_vis_per_s": n_vis / (grid_ms / 1e3),
@@ -449,7 +460,7 @@ def run_ours(args):
 def ncu_traffic(kernel, cfg, n_subgrids, launches_per_step):
     """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/), scaled from the
     captured launch to this run's average launch; None when there is no capture for this workload."""
-    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "dram_traffic_r01f.csv")
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "dram_traffic_r01g.csv")
     if cfg.config_id != 2 or not os.path.exists(path) or not launches_per_step:
         return None
     with open(path) as f:
