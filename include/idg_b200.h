@@ -177,6 +177,24 @@ IDG_API int  idg_splitter(const idg_plan* plan, int64_t first, int64_t count, co
 IDG_API int  idg_profile_enable(int on);
 IDG_API int  idg_profile_read(double* ms_out, int64_t* launches_out);
 
+/* ---- w-stacking closure either side of the path (Eq. 11 :145-148, Eq. 12 :164-166).
+ * NOT part of the measured hot path; the master-grid FFT is cuFFT's (its plan and work area are
+ * created on the first call and belong to the idg_plan).
+ *   idg_grid_to_image: image[p, y, x] = corr[y, x] * sum_layers e^{+2 pi i w0 n'(l_x, m_y)} *
+ *       sum_g grid[layer, p, g] e^{+2 pi i ((gy-Ng/2)(y-Ng/2) + (gx-Ng/2)(x-Ng/2)) / Ng}
+ *   idg_image_to_grid: grid[layer, p, g] = sum_j corr[j] e^{-2 pi i w0 n'_j} image[p, j] e^{-2 pi i (...)/Ng}
+ * w0 = (wl + 1/2) w_step (0 if w_step = 0), l_x = (x - Ng/2) S/Ng, no 1/Ng^2 factor in either direction.
+ * corr_dev: optional real [Ng, Ng] factor (NULL = 1), e.g. 1 / (T_full * n_vis) for a dirty image or
+ * 1 / T_full for a model (R4: the image-level taper correction is the caller's).
+ * grid_dev [n_wlayers, 4, Ng, Ng] c64, image_dev [4, Ng, Ng] c64 (overwritten / read),
+ * workspace_dev: idg_closure_workspace_bytes(plan) bytes for idg_grid_to_image (the grid is preserved);
+ * idg_image_to_grid overwrites grid_dev and needs no workspace. */
+IDG_API size_t idg_closure_workspace_bytes(const idg_plan* plan);
+IDG_API int  idg_grid_to_image(const idg_plan* plan, const void* grid_dev, const float* corr_dev, void* image_dev,
+                       void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
+IDG_API int  idg_image_to_grid(const idg_plan* plan, const void* image_dev, const float* corr_dev, void* grid_dev,
+                       void* cuda_stream);
+
 /* Kernel variant of the two direct-sum kernels (process-wide; kind = IDG_K_GRIDDER or
  * IDG_K_DEGRIDDER).  IDG_VARIANT_SIMT: all arithmetic on the FP32/SFU pipes (packed FFMA2).
  * IDG_VARIANT_TENSOR: the phasor matrix is generated on the SIMT pipes and the 2x2 complex MACs run

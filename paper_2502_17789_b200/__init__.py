@@ -25,6 +25,7 @@ SYMBOLS = (
     "idg_plan_create", "idg_plan_destroy", "idg_plan_counts", "idg_plan_export", "idg_workspace_bytes",
     "idg_grid", "idg_degrid", "idg_host_arena_bytes", "idg_grid_host", "idg_degrid_host",
     "idg_grid_subgrids", "idg_degrid_subgrids", "idg_subgrid_fft", "idg_adder", "idg_splitter",
+    "idg_closure_workspace_bytes", "idg_grid_to_image", "idg_image_to_grid",
     "idg_profile_enable", "idg_profile_read", "idg_set_kernel_variant", "idg_get_kernel_variant",
     "idg_measure_alu_peaks", "idg_launch_count", "idg_last_error", "idg_version",
 )
@@ -89,6 +90,12 @@ def load_library() -> ctypes.CDLL:
     lib.idg_adder.restype = ctypes.c_int
     lib.idg_splitter.argtypes = [vp, i64, i64, vp, vp, vp]
     lib.idg_splitter.restype = ctypes.c_int
+    lib.idg_closure_workspace_bytes.argtypes = [vp]
+    lib.idg_closure_workspace_bytes.restype = sz
+    lib.idg_grid_to_image.argtypes = [vp, vp, vp, vp, vp, sz, vp]
+    lib.idg_grid_to_image.restype = ctypes.c_int
+    lib.idg_image_to_grid.argtypes = [vp, vp, vp, vp, vp]
+    lib.idg_image_to_grid.restype = ctypes.c_int
     lib.idg_profile_enable.argtypes = [ctypes.c_int]
     lib.idg_profile_enable.restype = ctypes.c_int
     lib.idg_profile_read.argtypes = [vp, vp]
@@ -197,6 +204,9 @@ class Plan:
     def host_arena_bytes(self, direction=IDG_GRID) -> int:
         return int(load_library().idg_host_arena_bytes(self._h, direction))
 
+    def closure_workspace_bytes(self) -> int:
+        return int(load_library().idg_closure_workspace_bytes(self._h))
+
 
 def plan_from_config(cfg, uvw_m, freqs, baselines, max_batch_subgrids=0) -> Plan:
     """Convenience: a Plan from a `synth.Config`-like object (attribute names as in include/idg_b200.h)."""
@@ -212,6 +222,22 @@ def grid(plan: Plan, vis, aterms, taper, grid_out, workspace, stream=None) -> No
     _check(load_library().idg_grid(plan.handle, _ptr(vis), _ptr(aterms), _ptr(taper), _ptr(grid_out),
                                    _ptr(workspace), workspace.numel() * workspace.element_size(),
                                    _stream_ptr(stream)), "idg_grid")
+
+
+def grid_to_image(plan: Plan, grid_in, image_out, workspace, corr=None, stream=None) -> None:
+    """idg_grid_to_image (w-stacking closure, outside the hot path): image_out [4,Ng,Ng] complex64."""
+    _need_cuda(grid_in, image_out, workspace, *(() if corr is None else (corr,)))
+    _check(load_library().idg_grid_to_image(plan.handle, _ptr(grid_in), None if corr is None else _ptr(corr),
+                                            _ptr(image_out), _ptr(workspace),
+                                            workspace.numel() * workspace.element_size(), _stream_ptr(stream)),
+           "idg_grid_to_image")
+
+
+def image_to_grid(plan: Plan, image_in, grid_out, corr=None, stream=None) -> None:
+    """idg_image_to_grid: grid_out [W,4,Ng,Ng] complex64 is overwritten."""
+    _need_cuda(image_in, grid_out, *(() if corr is None else (corr,)))
+    _check(load_library().idg_image_to_grid(plan.handle, _ptr(image_in), None if corr is None else _ptr(corr),
+                                            _ptr(grid_out), _stream_ptr(stream)), "idg_image_to_grid")
 
 
 def degrid(plan: Plan, grid_in, aterms, taper, vis_out, workspace, stream=None) -> None:

@@ -19,7 +19,7 @@ INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libidg_b200.so")
 
-SOURCES = ["plan.cpp", "api.cu", "gridder.cu", "gridder_tc.cu", "degridder.cu", "degridder_tc.cu", "fft.cu", "adder.cu", "peaks.cu"]
+SOURCES = ["plan.cpp", "api.cu", "gridder.cu", "gridder_tc.cu", "degridder.cu", "degridder_tc.cu", "fft.cu", "adder.cu", "closure.cu", "peaks.cu"]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-ffp-contract=off", "-Xcompiler", "-fvisibility=hidden",
@@ -71,7 +71,8 @@ def build(force: bool = False, verbose: bool = False, extra_flags=(), out: str |
     tag = "" if out is None else "." + os.path.splitext(os.path.basename(out))[0]
     with concurrent.futures.ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
         objs = list(ex.map(lambda s: _compile(s, verbose, tuple(extra_flags), tag), SOURCES))
-    cmd = [_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", lib, *objs]
+    cmd = [_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", lib, *objs,
+           "-lcufft", "-Xlinker", "-rpath=/usr/local/cuda/lib64"]     # cuFFT: master-grid FFT of the closure only
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")

@@ -102,6 +102,7 @@ void free_device_state(DeviceState* d) {
   cudaFree(d->uvw); cudaFree(d->kappa); cudaFree(d->meta); cudaFree(d->nprime);
   for (auto& c : d->batch_csr) free_csr(&c);
   cudaFree(d->adder_partials); cudaFree(d->adder_counters);
+  closure_plan_destroy(d->closure_fft);
   delete d;
 }
 
@@ -582,6 +583,58 @@ int idg_degrid_host(const idg_plan* plan, const void* grid_host, const void* ate
   }
   IDG_CUDA(cudaStreamSynchronize(stream));
   IDG_CUDA(cudaStreamSynchronize(lane.s));
+  return IDG_OK;
+}
+
+// ---- w-stacking closure (outside the hot path) -------------------------------------------------
+namespace {
+int ensure_closure_fft(const idg_plan* plan, const DeviceState* d, void** out) {
+  std::lock_guard<std::mutex> lock(plan->mu);
+  DeviceState* dm = const_cast<DeviceState*>(d);
+  if (!dm->closure_fft && closure_plan_create(plan->par.grid_size, &dm->closure_fft) != 0) {
+    set_error("cuFFT plan creation failed for the master-grid transform");
+    return IDG_ECUDA;
+  }
+  *out = dm->closure_fft;
+  return IDG_OK;
+}
+}  // namespace
+
+size_t idg_closure_workspace_bytes(const idg_plan* plan) {
+  if (!plan) return 0;
+  const size_t Ng = plan->par.grid_size;
+  return 4 * Ng * Ng * sizeof(float2);
+}
+
+int idg_grid_to_image(const idg_plan* plan, const void* grid_dev, const float* corr_dev, void* image_dev,
+                      void* workspace_dev, size_t workspace_bytes, void* cuda_stream) {
+  if (!plan || !grid_dev || !image_dev) { set_error("idg_grid_to_image: null argument"); return IDG_EINVAL; }
+  if (!workspace_dev || workspace_bytes < idg_closure_workspace_bytes(plan)) {
+    set_error("idg_grid_to_image: workspace too small (see idg_closure_workspace_bytes)");
+    return IDG_ENOMEM;
+  }
+  const DeviceState* d = nullptr;
+  int rc = ensure_device(plan, &d);
+  if (rc != IDG_OK) return rc;
+  void* fft = nullptr;
+  if ((rc = ensure_closure_fft(plan, d, &fft)) != IDG_OK) return rc;
+  IDG_CUDA(launch_grid_to_image(fft, static_cast<const float2*>(grid_dev), corr_dev, static_cast<float2*>(image_dev),
+                                static_cast<float2*>(workspace_dev), plan->par.grid_size, plan->n_wlayers, plan->wl_min,
+                                plan->par.w_step, plan->image_size, static_cast<cudaStream_t>(cuda_stream)));
+  return IDG_OK;
+}
+
+int idg_image_to_grid(const idg_plan* plan, const void* image_dev, const float* corr_dev, void* grid_dev,
+                      void* cuda_stream) {
+  if (!plan || !grid_dev || !image_dev) { set_error("idg_image_to_grid: null argument"); return IDG_EINVAL; }
+  const DeviceState* d = nullptr;
+  int rc = ensure_device(plan, &d);
+  if (rc != IDG_OK) return rc;
+  void* fft = nullptr;
+  if ((rc = ensure_closure_fft(plan, d, &fft)) != IDG_OK) return rc;
+  IDG_CUDA(launch_image_to_grid(fft, static_cast<const float2*>(image_dev), corr_dev, static_cast<float2*>(grid_dev),
+                                plan->par.grid_size, plan->n_wlayers, plan->wl_min, plan->par.w_step, plan->image_size,
+                                static_cast<cudaStream_t>(cuda_stream)));
   return IDG_OK;
 }
 

@@ -52,6 +52,7 @@ struct DeviceState {
   std::vector<DeviceCsr> batch_csr;
   double* adder_partials = nullptr;   // shared by the batches: sized for the largest
   int32_t* adder_counters = nullptr;
+  void* closure_fft = nullptr;        // cuFFT plan of the master-grid transform, created on first use
   int device = -1;
 };
 

@@ -56,6 +56,15 @@ cudaError_t launch_adder(const int32_t* meta, const DeviceCsr& csr, int64_t firs
 cudaError_t launch_splitter(const int32_t* meta, int64_t first, int64_t count, int L, int Ng,
                             const float2* grid, float2* subgrids, cudaStream_t stream);
 
+// w-stacking closure (closure.cu; outside the hot path, master-grid FFT by cuFFT).  `fft_plan` comes from
+// closure_plan_create (one per idg_plan).  tmp: [4, Ng, Ng] complex64 scratch.
+int  closure_plan_create(int Ng, void** out);
+void closure_plan_destroy(void* fft_plan);
+cudaError_t launch_grid_to_image(void* fft_plan, const float2* grid, const float* corr, float2* image, float2* tmp,
+                                 int Ng, int n_layers, int wl_min, double w_step, double S, cudaStream_t stream);
+cudaError_t launch_image_to_grid(void* fft_plan, const float2* image, const float* corr, float2* grid, int Ng,
+                                 int n_layers, int wl_min, double w_step, double S, cudaStream_t stream);
+
 // Empirical FFMA / FFMA2 / MUFU rates per SM clock (peaks.cu); synchronous.
 cudaError_t measure_alu_peaks(double* out5);
 
