@@ -113,6 +113,13 @@ IDG_API size_t idg_workspace_bytes(const idg_plan* plan, int direction);
 IDG_API int  idg_grid(const idg_plan* plan, const void* vis_dev, const void* aterms_dev, const float* taper_dev,
               void* grid_dev, void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
 
+/* The same with imaging weights applied as the visibilities are loaded ("weighting ...
+ * performed by each thread"): vis[r, c, :] is multiplied by weights_dev[r, c]
+ * (float32 [n_rows, n_chan]; NULL = idg_grid).  Flagged samples are weight 0. */
+IDG_API int  idg_grid_weighted(const idg_plan* plan, const void* vis_dev, const float* weights_dev,
+                       const void* aterms_dev, const float* taper_dev, void* grid_dev, void* workspace_dev,
+                       size_t workspace_bytes, void* cuda_stream);
+
 /* ---- prediction direction, steps 3.i-3.iii of PAPER.md:168-174.  Writes vis_dev[r, c, :]
  * for every visibility covered by a subgrid and leaves the others untouched.  The same taper
  * array multiplies (R4) and the same sandwich M_p X M_q^H is applied (R5: pass A). */

@@ -23,7 +23,7 @@ STAGE_GRIDDER, STAGE_FFT = 0, 1
 # every symbol include/idg_b200.h declares
 SYMBOLS = (
     "idg_plan_create", "idg_plan_destroy", "idg_plan_counts", "idg_plan_export", "idg_workspace_bytes",
-    "idg_grid", "idg_degrid", "idg_host_arena_bytes", "idg_grid_host", "idg_degrid_host",
+    "idg_grid", "idg_grid_weighted", "idg_degrid", "idg_host_arena_bytes", "idg_grid_host", "idg_degrid_host",
     "idg_grid_subgrids", "idg_degrid_subgrids", "idg_subgrid_fft", "idg_adder", "idg_splitter",
     "idg_closure_workspace_bytes", "idg_grid_to_image", "idg_image_to_grid",
     "idg_profile_enable", "idg_profile_read", "idg_set_kernel_variant", "idg_get_kernel_variant",
@@ -74,6 +74,8 @@ def load_library() -> ctypes.CDLL:
     lib.idg_host_arena_bytes.restype = sz
     lib.idg_grid.argtypes = [vp, vp, vp, vp, vp, vp, sz, vp]
     lib.idg_grid.restype = ctypes.c_int
+    lib.idg_grid_weighted.argtypes = [vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.idg_grid_weighted.restype = ctypes.c_int
     lib.idg_degrid.argtypes = [vp, vp, vp, vp, vp, vp, sz, vp]
     lib.idg_degrid.restype = ctypes.c_int
     lib.idg_grid_host.argtypes = [vp, vp, vp, vp, vp, vp, sz, vp]
@@ -222,6 +224,15 @@ def grid(plan: Plan, vis, aterms, taper, grid_out, workspace, stream=None) -> No
     _check(load_library().idg_grid(plan.handle, _ptr(vis), _ptr(aterms), _ptr(taper), _ptr(grid_out),
                                    _ptr(workspace), workspace.numel() * workspace.element_size(),
                                    _stream_ptr(stream)), "idg_grid")
+
+
+def grid_weighted(plan: Plan, vis, weights, aterms, taper, grid_out, workspace, stream=None) -> None:
+    """idg_grid_weighted: as grid(), with vis[r, c, :] * weights[r, c] (float32) applied at load."""
+    _need_cuda(vis, weights, aterms, taper, grid_out, workspace)
+    _check(load_library().idg_grid_weighted(plan.handle, _ptr(vis), _ptr(weights), _ptr(aterms), _ptr(taper),
+                                            _ptr(grid_out), _ptr(workspace),
+                                            workspace.numel() * workspace.element_size(), _stream_ptr(stream)),
+           "idg_grid_weighted")
 
 
 def grid_to_image(plan: Plan, grid_in, image_out, workspace, corr=None, stream=None) -> None:

@@ -165,6 +165,7 @@ SubgridJob make_job(const idg_plan* plan, const DeviceState* d, int64_t first, i
   j.meta = d->meta; j.uvw = d->uvw; j.kappa = d->kappa; j.nprime = d->nprime;
   j.aterms = static_cast<const float4*>(aterms);
   j.taper = taper;
+  j.weights = nullptr;
   j.first = first; j.count = count;
   j.subgrid_size = plan->par.subgrid_size; j.grid_size = plan->par.grid_size;
   j.n_times = plan->par.n_times; j.n_chan = plan->par.n_chan; j.n_intervals = plan->n_intervals;
@@ -326,10 +327,11 @@ namespace {
 // between the FFT and the adder launches (the host-buffer call waits for the grid upload there).
 int grid_batch(const idg_plan* plan, const DeviceState* d, size_t i, const void* vis_dev, const void* aterms_dev,
                const float* taper_dev, void* grid_dev, float2* stack, cudaStream_t stream,
-               const std::function<int()>& before_adder) {
+               const std::function<int()>& before_adder, const float* weights_dev = nullptr) {
   const int L = plan->par.subgrid_size, Ng = plan->par.grid_size;
   const Batch& bt = plan->batches[i];
-  const SubgridJob job = make_job(plan, d, bt.first, bt.count, aterms_dev, taper_dev);
+  SubgridJob job = make_job(plan, d, bt.first, bt.count, aterms_dev, taper_dev);
+  job.weights = weights_dev;
   { ProfScope ps(IDG_K_GRIDDER, stream);
     IDG_CUDA(run_gridder(plan, job, static_cast<const float4*>(vis_dev), stack, stream)); }
   { ProfScope ps(IDG_K_FFT, stream);
@@ -358,8 +360,9 @@ int degrid_batch(const idg_plan* plan, const DeviceState* d, size_t i, const voi
 
 }  // namespace
 
-int idg_grid(const idg_plan* plan, const void* vis_dev, const void* aterms_dev, const float* taper_dev,
-             void* grid_dev, void* workspace_dev, size_t workspace_bytes, void* cuda_stream) {
+int idg_grid_weighted(const idg_plan* plan, const void* vis_dev, const float* weights_dev, const void* aterms_dev,
+                      const float* taper_dev, void* grid_dev, void* workspace_dev, size_t workspace_bytes,
+                      void* cuda_stream) {
   if (!plan || !vis_dev || !aterms_dev || !taper_dev || !grid_dev) { set_error("idg_grid: null argument"); return IDG_EINVAL; }
   if (plan->n_subgrids == 0) return IDG_OK;
   if (!workspace_dev || workspace_bytes < idg_workspace_bytes(plan, IDG_GRID)) {
@@ -372,10 +375,16 @@ int idg_grid(const idg_plan* plan, const void* vis_dev, const void* aterms_dev, 
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   for (size_t i = 0; i < plan->batches.size(); ++i) {
     rc = grid_batch(plan, d, i, vis_dev, aterms_dev, taper_dev, grid_dev, static_cast<float2*>(workspace_dev), stream,
-                    [] { return IDG_OK; });
+                    [] { return IDG_OK; }, weights_dev);
     if (rc != IDG_OK) return rc;
   }
   return IDG_OK;
+}
+
+int idg_grid(const idg_plan* plan, const void* vis_dev, const void* aterms_dev, const float* taper_dev,
+             void* grid_dev, void* workspace_dev, size_t workspace_bytes, void* cuda_stream) {
+  return idg_grid_weighted(plan, vis_dev, nullptr, aterms_dev, taper_dev, grid_dev, workspace_dev, workspace_bytes,
+                           cuda_stream);
 }
 
 int idg_degrid(const idg_plan* plan, const void* grid_dev, const void* aterms_dev, const float* taper_dev,

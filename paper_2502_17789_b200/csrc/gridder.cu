@@ -79,8 +79,13 @@ __global__ void __launch_bounds__(T) gridder_kernel(const SubgridJob job, const 
   auto stage_load = [&](int ci) {
     const int r = ci / cpr, cc = (ci % cpr) * kChunk;
     const int cnt = min(kChunk, nc - cc);
-    if (tid < 2 * cnt)
+    if (tid < 2 * cnt) {
       pre = __ldg(&vis[((row0 + r) * job.n_chan + c0 + cc) * 2 + tid]);
+      if (job.weights != nullptr) {                     // weighting at load
+        const float wgt = __ldg(&job.weights[(row0 + r) * job.n_chan + c0 + cc + (tid >> 1)]);
+        pre = make_float4(pre.x * wgt, pre.y * wgt, pre.z * wgt, pre.w * wgt);
+      }
+    }
   };
   auto stage_store = [&](int ci, int buf) {
     const int r = ci / cpr, cc = (ci % cpr) * kChunk;

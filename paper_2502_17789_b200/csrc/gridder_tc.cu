@@ -197,7 +197,13 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
       const int rr = ci / cpr;
       const int r = r_begin + rr, cc = (ci - rr * cpr) * KC;
       float2 v = make_float2(0.f, 0.f);
-      if (cc + j < nc) v = __ldg(reinterpret_cast<const float2*>(vis) + ((row0 + r) * job.n_chan + c0 + cc + j) * 4 + p);
+      if (cc + j < nc) {
+        v = __ldg(reinterpret_cast<const float2*>(vis) + ((row0 + r) * job.n_chan + c0 + cc + j) * 4 + p);
+        if (job.weights != nullptr) {                  // weighting at load
+          const float wgt = __ldg(&job.weights[(row0 + r) * job.n_chan + c0 + cc + j]);
+          v = make_float2(v.x * wgt, v.y * wgt);
+        }
+      }
       const float hr = tf32_round(v.x), hi = tf32_round(v.y);
       const float lr = tf32_round(v.x - hr), li = tf32_round(v.y - hi);
       float* Bf = reinterpret_cast<float*>(sB + static_cast<size_t>(ci) * CHUNK_BYTES);

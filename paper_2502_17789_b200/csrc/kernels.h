@@ -17,6 +17,7 @@ struct SubgridJob {
   const float* nprime;      // [L, L] n'(l, m) at the subgrid pixels
   const float4* aterms;     // [n_st, n_int, L, L, 2] rows of the 2x2 Jones matrices
   const float* taper;       // [L, L]
+  const float* weights;     // [n_rows, n_chan] imaging weights applied at load, or nullptr
   int64_t first;            // first subgrid (global index)
   int64_t count;
   int32_t subgrid_size, grid_size, n_times, n_chan, n_intervals;

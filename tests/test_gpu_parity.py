@@ -378,3 +378,23 @@ def test_full_size_config2_sampled(idg):
         r0 = b * cfg.n_times + t0
         e = nerr(out[r0:r0 + nt, c0:c0 + nc], ref)
         assert e <= TOL, (s, sub[s].tolist(), e)
+
+
+@pytest.mark.parametrize("variant", ["simt", "tensor"])
+def test_weighted_gridding(idg, variant):
+    """SURVEY §8(f) NEXT-2, weights at load: idg_grid_weighted == the oracle on vis * weights,
+    zero weights (flags) included."""
+    request_variant(idg, variant, kind="gridder")
+    cfg = synth.scaled(synth.get_config(2), n_stations=7, n_times=16, grid_size=1024, cell_arcsec=120.0)
+    obs, par, plan, sub = setup(idg, cfg, vis="hash")
+    cnt = plan.counts()
+    rng = np.random.default_rng(21)
+    wgt = rng.uniform(0.0, 2.0, (cfg.n_rows, cfg.n_chan)).astype(np.float32)
+    wgt[rng.random(wgt.shape) < 0.1] = 0.0
+    Ng = cfg.grid_size
+    d_grid = torch.zeros((cnt.n_wlayers, 4, Ng, Ng), dtype=torch.complex64, device=DEV)
+    ws = torch.empty(plan.workspace_bytes(), dtype=torch.uint8, device=DEV)
+    idg.grid_weighted(plan, dev(obs.vis), dev(wgt), dev(obs.aterms), dev(obs.taper), d_grid, ws)
+    ref = orc.grid(par, sub, obs.uvw, obs.freqs, obs.vis.astype(np.complex128) * wgt[:, :, None].astype(np.float64),
+                   obs.baselines, obs.aterms, obs.taper)
+    assert nerr(d_grid.cpu().numpy(), ref) <= TOL
