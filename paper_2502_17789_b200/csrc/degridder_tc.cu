@@ -287,17 +287,19 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
       // cl = chunks left in my share of the current stage; kept in plain registers (`opaque`)
       const int ncs_r = static_cast<int>(tc::opaque(static_cast<uint32_t>(ncs)));
       const int lp0 = static_cast<int>(tc::opaque(static_cast<uint32_t>((part << lgn) * kKC)));
-      int left = total, cl = 0, st = 0, rig = 0, gin = 0;
+      int cl = 0, st = 0, rig = 0, gin = 0;
       for (int rev = 0; rev < nrev; ++rev) {
 #pragma unroll
         for (int s = 0; s < NA; ++s) {
-          const bool valid = left > 0;
+          // slots past the round's last chunk are computed and stored like any other (the service warp issues
+          // no MMA for them), so the compute threads never test whether a slot is in use
+          constexpr bool valid = true;
           // the previous slot goes to the service warp before this one's arithmetic
           if (s > 0) hand_off(gbar + 8 * (s - 1));
           else if (pending) hand_off(gbar + 8 * (NA - 1));
           uint32_t hi[16], lo[16];
           if (valid) {
-            if (cl == 0) {
+            if (cl == 0 && st < NSTAGES) {
               // a new stage: wait for the producer, find my share of its pixels
               const int gst = sc0 + st, slot = gst & (NS - 1);
               tc::mbar_wait(bar_sfull + 8 * slot, (gst / NS) & 1);
@@ -339,7 +341,6 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
           if (valid) {
             tc::tmem_st16(gtmem + s * A_COLS, hi);
             tc::tmem_st16(gtmem + s * A_COLS + 2 * kKC, lo);
-            --left;
             np_addr += kKC * 4;
             fx0 += static_cast<float>(kKC);
             if (fx0 >= static_cast<float>(L / 2)) { fx0 = static_cast<float>(-L / 2); fy += 1.f; }

@@ -192,12 +192,15 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
     if (seg > 0) __syncthreads();                      // every MMA of the previous segment was drained
     // One warp per 8 visibilities x 4 polarisations, so the row / channel split is once per warp.
     constexpr int UPC = KC / 8;
-    for (int u = warp; u < nchunks * UPC; u += NTHREADS / 32) {
+    // the chunk count is padded to whole ring revolutions with zero chunks (B = 0 contributes nothing), so
+    // neither the compute threads nor the service warp ever test whether a slot is in use
+    const int nchunks_pad = (nchunks + NA - 1) / NA * NA;
+    for (int u = warp; u < nchunks_pad * UPC; u += NTHREADS / 32) {
       const int ci = u / UPC, j = (u % UPC) * 8 + ((tid & 31) >> 2), p = tid & 3;
       const int rr = ci / cpr;
       const int r = r_begin + rr, cc = (ci - rr * cpr) * KC;
       float2 v = make_float2(0.f, 0.f);
-      if (cc + j < nc) {
+      if (ci < nchunks && cc + j < nc) {
         v = __ldg(reinterpret_cast<const float2*>(vis) + ((row0 + r) * job.n_chan + c0 + cc + j) * 4 + p);
         if (job.weights != nullptr) {                  // weighting at load
           const float wgt = __ldg(&job.weights[(row0 + r) * job.n_chan + c0 + cc + j]);
@@ -244,14 +247,12 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
             tc::fence_after_thread_sync();
             const uint64_t bdesc0 = tc::make_smem_desc(bbase + ci * CHUNK_BYTES, 256, 128);
             if (tc::elect_one()) {
-              if (ci < n_u) {
 #pragma unroll
-                for (int part = 0; part < 2; ++part)
+              for (int part = 0; part < 2; ++part)
 #pragma unroll
-                  for (int ks = 0; ks < KC / 4; ++ks)
-                    tc::mma_tf32_ts(d0, gt + s * A_COLS + part * 2 * KC + ks * 8, bdesc0 + ks * (512 >> 4), IDESC,
-                                    (rig > 0 || s > 0 || part > 0 || ks > 0) ? 1u : 0u);
-              }
+                for (int ks = 0; ks < KC / 4; ++ks)
+                  tc::mma_tf32_ts(d0, gt + s * A_COLS + part * 2 * KC + ks * 8, bdesc0 + ks * (512 >> 4), IDESC,
+                                  (rig > 0 || s > 0 || part > 0 || ks > 0) ? 1u : 0u);
               tc::mma_commit(sbar + 8 * NA + 8 * s);
               if (s == NA - 1 && group_last) tc::mma_commit(sbar + 16 * NA + 8 * (q & 1));
             }
@@ -326,11 +327,10 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
         row_setup(r);
         uint32_t dk_addr = sdk_addr;
         int rig = 0, gin = 0;                          // revolutions in the current group, groups closed in this tile
-        int left = nchunks;                            // chunks of this tile still to store
         for (int rev = 0; rev < nrev; ++rev) {
 #pragma unroll
           for (int s = 0; s < NA; ++s) {
-            const bool valid = left > 0;
+            constexpr bool valid = true;                // padding chunks are computed like any other
             // the previous slot goes to the service warp before this one's arithmetic: its stores were
             // issued a whole hand-off / wait / store sequence ago
             if (s > 0) hand_off(gbar + 8 * (s - 1));
@@ -372,7 +372,6 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
                 tc::tmem_st16(gtmem + s * A_COLS + half * 16, hi[half]);
                 tc::tmem_st16(gtmem + s * A_COLS + 2 * KC + half * 16, lo[half]);
               }
-              --left;
               dk_addr += KC * 4;
               cc += KC;
               if (cc >= nc) {
@@ -419,11 +418,12 @@ cudaError_t launch(const SubgridJob& job, const float4* vis, float2* out, cudaSt
   constexpr int CHUNK_BYTES = KC * 128;
   const int cpr_max = (job.n_chan + KC - 1) / KC;
   const int cap_chunks = std::min(job.max_nt * cpr_max, kMaxBBytes / CHUNK_BYTES);
-  const size_t dyn = static_cast<size_t>(cap_chunks) * CHUNK_BYTES;
+  const size_t dyn = static_cast<size_t>(cap_chunks + NA - 1) * CHUNK_BYTES;   // + padding chunks
   auto kernel = gridder_tc_kernel<L, NG, KC, DG, NA>;
   static size_t configured = 0;                        // per instantiation
   if (dyn > configured) {
-    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxBBytes);
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         kMaxBBytes + (NA - 1) * CHUNK_BYTES);
     if (e != cudaSuccess) return e;
     configured = kMaxBBytes;
   }
@@ -439,7 +439,7 @@ cudaError_t launch(const SubgridJob& job, const float4* vis, float2* out, cudaSt
 template <int L>
 cudaError_t launch_l(const SubgridJob& job, const float4* vis, float2* out, cudaStream_t stream) {
   constexpr int KC = IDG_TC_KC;
-  const size_t dyn = static_cast<size_t>(std::min(job.max_nt * ((job.n_chan + KC - 1) / KC), kMaxBBytes / (KC * 128))) *
+  const size_t dyn = static_cast<size_t>(std::min(job.max_nt * ((job.n_chan + KC - 1) / KC), kMaxBBytes / (KC * 128)) + IDG_TC_NA - 1) *
                      (KC * 128);
   constexpr size_t kStaticAndReserved = 11 * 1024, kSmemPerSm = 227 * 1024;
 #ifdef IDG_TC_NG
