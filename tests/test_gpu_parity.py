@@ -47,6 +47,9 @@ CASES = [
      "hash"),
     ("wide-rows", lambda: synth.scaled(synth.get_config(1), n_stations=5, n_times=8, n_chan=150, chan_width_hz=2e3),
      "hash"),
+    # more channels than the tensor-core gridder's tables hold: it must hand the launch to the SIMT kernel
+    ("many-chan", lambda: synth.scaled(synth.get_config(1), n_stations=3, n_times=4, n_chan=1300, chan_width_hz=150.0),
+     "hash"),
     # more visibilities per subgrid than the tensor-core gridder keeps in shared memory: segmented path
     ("long-rows", lambda: synth.scaled(synth.get_config(1), n_stations=4, n_times=8, n_chan=220, chan_width_hz=1e3),
      "hash"),
