@@ -369,8 +369,12 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
             if (valid) {
 #pragma unroll
               for (int half = 0; half < KC / 8; ++half) {
-                tc::tmem_st16(gtmem + s * A_COLS + half * 16, hi[half]);
-                tc::tmem_st16(gtmem + s * A_COLS + 2 * KC + half * 16, lo[half]);
+                if constexpr (KC == 8) {
+                  tc::tmem_st32(gtmem + s * A_COLS, hi[half], lo[half]);     // heads and remainders are adjacent
+                } else {
+                  tc::tmem_st16(gtmem + s * A_COLS + half * 16, hi[half]);
+                  tc::tmem_st16(gtmem + s * A_COLS + 2 * KC + half * 16, lo[half]);
+                }
               }
               dk_addr += KC * 4;
               cc += KC;
