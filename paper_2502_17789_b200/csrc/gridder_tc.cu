@@ -11,13 +11,21 @@
 // part, 8 pairs/clk/SM) and hand it to the tensor cores through tensor memory; the 16 FMAs per pair
 // that bound a SIMT kernel at 7.11 pairs/clk/SM leave the FP32 pipe.
 //
-// Precision.  kind::tf32 keeps 11 significant bits, so every operand is split into a tf32-exact head
-// and an fp32 remainder: E = Eh + El (mask + exact subtraction), V = Vh + Vl.  One MMA of N = 16
-// columns [B(Vh) | B(Vl)] per A part gives Eh Vh + Eh Vl + El Vh + El Vl; the two column halves are
-// added when the accumulator is read.  The tensor core's fp32 accumulation truncates, which biases
-// long chains (measured 4e-6 after 128 MMAs), so the accumulator is drained into fp32 registers
-// (round-to-nearest adds) every DG chunks, alternating two TMEM accumulators so that draining one
-// overlaps the MMAs into the other.
+// Precision.  The tensor core takes 11-bit operands (fp16 and tf32 alike), so every operand is split into a
+// head and a remainder: E = Eh + El, V = Vh + Vl.  Default (IDG_TC_FP16): fp16 heads and fp16 remainders.
+// |E| <= 1, so (cos, sin) of one visibility pack into ONE 32-bit word of heads and one of remainders, 8 B per
+// (visibility, pixel) pair in tensor memory instead of 16, and a chunk of 8 visibilities is one K = 16
+// kind::f16 MMA per part instead of two K = 8 kind::tf32 ones; the remainder (<= 2^-12) is kept to 2^-25
+// absolute.  The visibilities are brought into fp16's range by one power-of-two scale per segment (the largest
+// |component|, found while staging), undone exactly when a tile is finished.  -DIDG_TC_TF32 selects the first
+// scheme instead: tf32-exact heads by masking, fp32 remainders, 16 B per pair.  Either way one MMA of N = 16
+// columns [B(Vh) | B(Vl)] per A part gives Eh Vh + Eh Vl + El Vh + El Vl, the two column halves being added
+// when the accumulator is read.  The tensor core's fp32 accumulation truncates, which biases long chains, so
+// the accumulator is drained into fp32 registers (round-to-nearest adds) every DG chunks, alternating two TMEM
+// accumulators so that draining one overlaps the MMAs into the other.  Measured against the oracle: 1.1e-6
+// per subgrid and 0.8e-6 on a recovered point-source flux (fp16, DG = 12: 24 MMAs per accumulator); 1.7e-6 and
+// 1.8e-6 with tf32 operands (48 MMAs).  Halving the bytes stored per pair is also why it is faster (the
+// tensor-memory stores cost 20 % of the tf32 kernel's time): 5.45 against 5.19 pairs/clk/SM on config 2.
 //
 // One CTA per subgrid: NG groups of 128 compute threads plus one service warp per group; NG = 1, 2 or 4
 // chosen at launch so that 4 / NG CTAs share an SM (see launch_l).
@@ -37,6 +45,8 @@
 //                    accumulator group's end, to dfull[group][q & 1].
 #include <algorithm>
 
+#include <cuda_fp16.h>
+
 #include "device_math.cuh"
 #include "kernels.h"
 #include "tc_common.cuh"
@@ -45,6 +55,9 @@ namespace idg {
 
 namespace {
 
+#ifndef IDG_TC_TF32
+#define IDG_TC_FP16 1                 // operand format: fp16 head + fp16 remainder (default) or split tf32
+#endif
 #ifndef IDG_TC_KC
 #define IDG_TC_KC 8
 #endif
@@ -52,7 +65,11 @@ namespace {
 #define IDG_TC_DG 12
 #endif
 #ifndef IDG_TC_NA
+#ifdef IDG_TC_FP16
+#define IDG_TC_NA 4
+#else
 #define IDG_TC_NA 3
+#endif
 #endif
 
 constexpr int kTileM = 128;           // pixels per MMA tile = threads per compute group
@@ -67,8 +84,8 @@ struct RowDataTc {
 };
 
 // tf32-exact head of x (the low 13 mantissa bits cleared); x - head is exact in fp32
-__device__ __forceinline__ float tf32_head(float x) { return __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
-__device__ __forceinline__ float tf32_round(float x) {
+[[maybe_unused]] __device__ __forceinline__ float tf32_head(float x) { return __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
+[[maybe_unused]] __device__ __forceinline__ float tf32_round(float x) {
   return __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
 }
 
@@ -82,22 +99,36 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
   static_assert(TILES % NG == 0 && (KC == 8 || KC == 16) && NA >= 2, "shape");
   constexpr int ROUNDS = TILES / NG;
   constexpr int NTHREADS = NG * kTileM + NG * 32;
+#ifdef IDG_TC_FP16
+  static_assert(KC == 8, "fp16 operands: 8-channel chunks");
+  constexpr int A_COLS = 2 * KC;                       // per slot: 8 words of (cos, sin) heads, 8 of remainders
+#else
   constexpr int A_COLS = 4 * KC;                       // per slot: heads [0, 2KC), remainders [2KC, 4KC)
+#endif
   constexpr int D_COL = NA * A_COLS;                   // then two accumulators of 16 columns
   constexpr int GCOLS = D_COL + 32;                    // TMEM columns per compute group
   constexpr int TMEM_COLS = NG * GCOLS <= 128 ? 128 : (NG * GCOLS <= 256 ? 256 : 512);
   static_assert(NG * GCOLS <= 512, "TMEM");
+#ifdef IDG_TC_FP16
+  constexpr int CHUNK_BYTES = KC * 64;                 // 2 KC k-rows x 16 columns x 2 bytes
+#else
   constexpr int CHUNK_BYTES = KC * 128;                // 2 KC k-rows x 16 columns x 4 bytes
+#endif
   static_assert(DG % NA == 0, "an accumulator group is a whole number of ring revolutions");
   constexpr int RPG = DG / NA;                         // revolutions per accumulator group
   constexpr int NBAR = 2 * NA + 4;                     // per group: full[NA], empty[NA], dfull[2], dempty[2]
+#ifdef IDG_TC_FP16
+  constexpr uint32_t IDESC = tc::make_idesc_f16(kTileM, 16);
+#else
   constexpr uint32_t IDESC = tc::make_idesc_tf32(kTileM, 16);
+#endif
 
   extern __shared__ __align__(1024) unsigned char sB[];   // [cap_chunks][CHUNK_BYTES]
   __shared__ __align__(16) float sdk[kMaxChanTc];
   __shared__ RowDataTc srow[kMaxRowsTc];
   __shared__ __align__(8) uint64_t bars[NG * NBAR];
   __shared__ uint32_t s_tmem;
+  __shared__ uint32_t s_vmax;                          // fp16 operands: bits of the segment's largest |component|
 
   const int tid = threadIdx.x, warp = tid / 32;
   const int64_t sg = blockIdx.x;
@@ -195,6 +226,60 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
     // the chunk count is padded to whole ring revolutions with zero chunks (B = 0 contributes nothing), so
     // neither the compute threads nor the service warp ever test whether a slot is in use
     const int nchunks_pad = (nchunks + NA - 1) / NA * NA;
+#ifdef IDG_TC_FP16
+    // fp16 operands need the visibilities in range: one power-of-two scale per segment, undone at the drain
+    if (tid == 0) s_vmax = 0u;
+    __syncthreads();
+    {
+      float mx = 0.f;
+      for (int u = warp; u < nchunks * UPC; u += NTHREADS / 32) {
+        const int ci = u / UPC, j = (u % UPC) * 8 + ((tid & 31) >> 2), p = tid & 3;
+        const int rr = ci / cpr;
+        const int r = r_begin + rr, cc = (ci - rr * cpr) * KC;
+        if (cc + j < nc) {
+          float2 v = __ldg(reinterpret_cast<const float2*>(vis) + ((row0 + r) * job.n_chan + c0 + cc + j) * 4 + p);
+          if (job.weights != nullptr) {
+            const float wgt = __ldg(&job.weights[(row0 + r) * job.n_chan + c0 + cc + j]);
+            v = make_float2(v.x * wgt, v.y * wgt);
+          }
+          mx = fmaxf(mx, fmaxf(fabsf(v.x), fabsf(v.y)));
+        }
+      }
+      for (int o2 = 16; o2 > 0; o2 >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o2));
+      if ((tid & 31) == 0) atomicMax(&s_vmax, __float_as_uint(mx));
+    }
+    __syncthreads();
+    // scale = 2^e >= max, so every component / scale lies in [-1, 1]
+    const uint32_t ebits = (s_vmax & 0x7f800000u);
+    const float vscale = ebits == 0u ? 1.f : __uint_as_float(ebits + 0x00800000u);
+    const float vinv = 1.f / vscale;
+    for (int u = warp; u < nchunks_pad * UPC; u += NTHREADS / 32) {
+      const int ci = u / UPC, j = (u % UPC) * 8 + ((tid & 31) >> 2), p = tid & 3;
+      const int rr = ci / cpr;
+      const int r = r_begin + rr, cc = (ci - rr * cpr) * KC;
+      float2 v = make_float2(0.f, 0.f);
+      if (ci < nchunks && cc + j < nc) {
+        v = __ldg(reinterpret_cast<const float2*>(vis) + ((row0 + r) * job.n_chan + c0 + cc + j) * 4 + p);
+        if (job.weights != nullptr) {
+          const float wgt = __ldg(&job.weights[(row0 + r) * job.n_chan + c0 + cc + j]);
+          v = make_float2(v.x * wgt, v.y * wgt);
+        }
+        v = make_float2(v.x * vinv, v.y * vinv);
+      }
+      const __half hr = __float2half_rn(v.x), hi = __float2half_rn(v.y);
+      const __half lr = __float2half_rn(v.x - __half2float(hr)), li = __float2half_rn(v.y - __half2float(hi));
+      // element (n, k) of the chunk's N x K operand: ((k/8)*2 + n/8)*128 + (n%8)*16 + (k%8)*2 bytes, k = 2 j + part
+      unsigned char* Bc = sB + static_cast<size_t>(ci) * CHUNK_BYTES;
+      auto at2 = [&](int n) -> __half2* {
+        return reinterpret_cast<__half2*>(Bc + ((j >> 2) * 2 + (n >> 3)) * 128 + (n & 7) * 16 + (j & 3) * 4);
+      };
+      *at2(2 * p) = __halves2half2(hr, __hneg(hi));     // column (p,re): rows (v,cos) = Re V, (v,sin) = -Im V
+      *at2(2 * p + 1) = __halves2half2(hi, hr);         // column (p,im): rows (v,cos) = Im V, (v,sin) =  Re V
+      *at2(2 * p + 8) = __halves2half2(lr, __hneg(li));
+      *at2(2 * p + 9) = __halves2half2(li, lr);
+    }
+#else
+    const float vscale = 1.f;
     for (int u = warp; u < nchunks_pad * UPC; u += NTHREADS / 32) {
       const int ci = u / UPC, j = (u % UPC) * 8 + ((tid & 31) >> 2), p = tid & 3;
       const int rr = ci / cpr;
@@ -218,6 +303,7 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
       *at2(2 * p + 8) = make_float2(lr, -li);
       *at2(2 * p + 9) = make_float2(li, lr);
     }
+#endif
     tc::fence_proxy_async();
     __syncthreads();
 
@@ -247,12 +333,18 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
             tc::fence_after_thread_sync();
             const uint64_t bdesc0 = tc::make_smem_desc(bbase + ci * CHUNK_BYTES, 256, 128);
             if (tc::elect_one()) {
+#ifdef IDG_TC_FP16
+#pragma unroll
+              for (int part = 0; part < 2; ++part)      // heads, remainders: one K = 16 MMA each
+                tc::mma_f16_ts(d0, gt + s * A_COLS + part * KC, bdesc0, IDESC, (rig > 0 || s > 0 || part > 0) ? 1u : 0u);
+#else
 #pragma unroll
               for (int part = 0; part < 2; ++part)
 #pragma unroll
                 for (int ks = 0; ks < KC / 4; ++ks)
                   tc::mma_tf32_ts(d0, gt + s * A_COLS + part * 2 * KC + ks * 8, bdesc0 + ks * (512 >> 4), IDESC,
                                   (rig > 0 || s > 0 || part > 0 || ks > 0) ? 1u : 0u);
+#endif
               tc::mma_commit(sbar + 8 * NA + 8 * s);
               if (s == NA - 1 && group_last) tc::mma_commit(sbar + 16 * NA + 8 * (q & 1));
             }
@@ -284,7 +376,7 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
       auto finalize = [&](const float (&a)[8], int pix) {
         float2 x[4], z[4];
 #pragma unroll
-        for (int p = 0; p < 4; ++p) x[p] = make_float2(a[2 * p], a[2 * p + 1]);
+        for (int p = 0; p < 4; ++p) x[p] = make_float2(a[2 * p] * vscale, a[2 * p + 1] * vscale);
         if (!first_seg) {
 #pragma unroll
           for (int p = 0; p < 4; ++p) {
@@ -351,6 +443,18 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
                   float2 e0, e1;                        // (cos, sin) of the two phases
                   __sincosf(ph.x, &e0.y, &e0.x);
                   __sincosf(ph.y, &e1.y, &e1.x);
+#ifdef IDG_TC_FP16
+                  // (cos, sin) -> fp16 head pair and fp16 remainder pair, one 32-bit word each
+                  const __half2 q0 = __floats2half2_rn(e0.x, e0.y), q1 = __floats2half2_rn(e1.x, e1.y);
+                  const float2 f0 = __half22float2(q0), f1 = __half22float2(q1);
+                  const float2 m1 = make_float2(-1.f, -1.f);
+                  const float2 l0 = ffma2(f0, m1, e0), l1 = ffma2(f1, m1, e1);
+                  const __half2 r0 = __floats2half2_rn(l0.x, l0.y), r1 = __floats2half2_rn(l1.x, l1.y);
+                  hi[half][2 * j2] = *reinterpret_cast<const uint32_t*>(&q0);
+                  hi[half][2 * j2 + 1] = *reinterpret_cast<const uint32_t*>(&q1);
+                  hi[half][8 + 2 * j2] = *reinterpret_cast<const uint32_t*>(&r0);
+                  hi[half][8 + 2 * j2 + 1] = *reinterpret_cast<const uint32_t*>(&r1);
+#else
                   const float2 h0 = make_float2(tf32_head(e0.x), tf32_head(e0.y));
                   const float2 h1 = make_float2(tf32_head(e1.x), tf32_head(e1.y));
                   const float2 l0 = ffma2(h0, m1, e0), l1 = ffma2(h1, m1, e1);      // e - head, exact
@@ -362,6 +466,7 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
                   lo[half][4 * j2 + 1] = __float_as_uint(l0.y);
                   lo[half][4 * j2 + 2] = __float_as_uint(l1.x);
                   lo[half][4 * j2 + 3] = __float_as_uint(l1.y);
+#endif
                 }
               }
             }
@@ -370,7 +475,11 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
 #pragma unroll
               for (int half = 0; half < KC / 8; ++half) {
                 if constexpr (KC == 8) {
+#ifdef IDG_TC_FP16
+                  tc::tmem_st16(gtmem + s * A_COLS, hi[half]);               // 8 head words, 8 remainder words
+#else
                   tc::tmem_st32(gtmem + s * A_COLS, hi[half], lo[half]);     // heads and remainders are adjacent
+#endif
                 } else {
                   tc::tmem_st16(gtmem + s * A_COLS + half * 16, hi[half]);
                   tc::tmem_st16(gtmem + s * A_COLS + 2 * KC + half * 16, lo[half]);
@@ -419,7 +528,11 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
 template <int L, int NG, int KC, int DG, int NA>
 cudaError_t launch(const SubgridJob& job, const float4* vis, float2* out, cudaStream_t stream) {
   if (job.count == 0) return cudaSuccess;
+#ifdef IDG_TC_FP16
+  constexpr int CHUNK_BYTES = KC * 64;
+#else
   constexpr int CHUNK_BYTES = KC * 128;
+#endif
   const int cpr_max = (job.n_chan + KC - 1) / KC;
   const int cap_chunks = std::min(job.max_nt * cpr_max, kMaxBBytes / CHUNK_BYTES);
   const size_t dyn = static_cast<size_t>(cap_chunks + NA - 1) * CHUNK_BYTES;   // + padding chunks
