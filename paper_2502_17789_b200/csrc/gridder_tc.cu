@@ -76,6 +76,11 @@ constexpr int kTileM = 128;           // pixels per MMA tile = threads per compu
 constexpr int kMaxRowsTc = 128;       // rows of one subgrid whose constants are kept in shared memory
 constexpr int kMaxChanTc = 1280;      // channels of one subgrid whose offsets are kept in shared memory
 constexpr int kMaxBBytes = 160 * 1024;   // shared memory for the B operand
+#ifdef IDG_TC_FP16
+constexpr int kVisBytes = 64;            // B operand bytes per visibility: 2 k-rows x 16 columns x 2 bytes
+#else
+constexpr int kVisBytes = 128;           // 2 k-rows x 16 columns x 4 bytes
+#endif
 
 struct RowDataTc {
   int32_t alpha_fix, beta_fix;   // (u-u0) S/L and (v-v0) S/L at kappa_ref, cycles/pixel * 2^32 (wrapping)
@@ -556,8 +561,8 @@ cudaError_t launch(const SubgridJob& job, const float4* vis, float2* out, cudaSt
 template <int L>
 cudaError_t launch_l(const SubgridJob& job, const float4* vis, float2* out, cudaStream_t stream) {
   constexpr int KC = IDG_TC_KC;
-  const size_t dyn = static_cast<size_t>(std::min(job.max_nt * ((job.n_chan + KC - 1) / KC), kMaxBBytes / (KC * 128)) + IDG_TC_NA - 1) *
-                     (KC * 128);
+  const size_t dyn = static_cast<size_t>(std::min(job.max_nt * ((job.n_chan + KC - 1) / KC), kMaxBBytes / (KC * kVisBytes)) + IDG_TC_NA - 1) *
+                     (KC * kVisBytes);
   constexpr size_t kStaticAndReserved = 11 * 1024, kSmemPerSm = 227 * 1024;
 #ifdef IDG_TC_NG
   return launch<L, IDG_TC_NG, KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
@@ -574,7 +579,7 @@ cudaError_t launch_gridder_tc(const SubgridJob& job, const float4* vis, float2* 
   // shapes whose per-subgrid constants do not fit the kernel's shared-memory tables take the SIMT kernel
   constexpr int KC = IDG_TC_KC;
   if (job.n_chan > kMaxChanTc - KC || job.max_nt > kMaxRowsTc ||
-      (job.n_chan + KC - 1) / KC > kMaxBBytes / (KC * 128))
+      (job.n_chan + KC - 1) / KC > kMaxBBytes / (KC * kVisBytes))
     return launch_gridder(job, vis, out, stream);
   switch (job.subgrid_size) {
     case 32:  return launch_l<32>(job, vis, out, stream);
