@@ -128,8 +128,8 @@ IDG_API int  idg_degrid(const idg_plan* plan, const void* grid_dev, const void* 
 
 /* ---- the same two calls on HOST buffers (pinned memory recommended: pageable memory makes the
  * copies synchronous).  They copy the inputs to `arena_dev`, run the device path on `cuda_stream`,
- * copy the result back (grid_host is accumulated into: it is uploaded too) and synchronise before
- * returning.  Copies run on a second stream and overlap compute batch by batch: a visibility row
+ * copy the result back (grid_host is accumulated into: it is uploaded behind the visibilities and added
+ * on the device after the subgrids) and synchronise before returning.  Copies run on a second stream and overlap compute batch by batch: a visibility row
  * goes up just before the first batch that reads it and comes down right after the last batch
  * that writes it, so a plan with smaller batches (idg_params.max_batch_subgrids) overlaps more.
  * idg_degrid_host uploads vis_host only when the planner left visibilities uncovered (they come

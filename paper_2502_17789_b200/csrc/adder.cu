@@ -178,7 +178,24 @@ __global__ void __launch_bounds__(256) splitter_kernel(const int32_t* __restrict
   }
 }
 
+// dst += src (the host-buffer imaging call adds the caller's grid after the subgrids, off the critical path)
+__global__ void __launch_bounds__(256) grid_add_kernel(const float2* __restrict__ src, float2* __restrict__ dst,
+                                                       int64_t n) {
+  for (int64_t i = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x; i < n;
+       i += static_cast<int64_t>(gridDim.x) * blockDim.x) {
+    const float2 a = src[i], b = dst[i];
+    dst[i] = make_float2(a.x + b.x, a.y + b.y);
+  }
+}
+
 }  // namespace
+
+cudaError_t launch_grid_add(const float2* src, float2* dst, int64_t n, cudaStream_t stream) {
+  if (n == 0) return cudaSuccess;
+  grid_add_kernel<<<148 * 8, 256, 0, stream>>>(src, dst, n);
+  count_launch();
+  return cudaGetLastError();
+}
 
 cudaError_t launch_adder(const int32_t* meta, const DeviceCsr& csr, int64_t first, int L, int Ng, int tiles_x,
                          int tiles_y, const float2* subgrids, float2* grid, cudaStream_t stream) {

@@ -408,9 +408,9 @@ int idg_degrid(const idg_plan* plan, const void* grid_dev, const void* aterms_de
 
 // ---- host-buffer variants -------------------------------------------------------------------
 namespace {
-struct ArenaLayout { size_t vis, aterms, taper, grid, work, total; };
+struct ArenaLayout { size_t vis, aterms, taper, grid, grid_in, work, total; };
 size_t align_up(size_t x) { return (x + 255) & ~size_t{255}; }
-ArenaLayout arena_layout(const idg_plan* plan) {
+ArenaLayout arena_layout(const idg_plan* plan, int direction = IDG_GRID) {
   const idg_params& p = plan->par;
   const size_t L = p.subgrid_size, Ng = p.grid_size;
   ArenaLayout a{};
@@ -419,6 +419,8 @@ ArenaLayout arena_layout(const idg_plan* plan) {
   a.aterms = off; off += align_up(static_cast<size_t>(p.n_stations) * plan->n_intervals * L * L * 4 * sizeof(float2));
   a.taper = off;  off += align_up(L * L * sizeof(float));
   a.grid = off;   off += align_up(static_cast<size_t>(plan->n_wlayers) * 4 * Ng * Ng * sizeof(float2));
+  // imaging only: the caller's grid waits here until the subgrids have been added (see idg_grid_host)
+  a.grid_in = off; if (direction == IDG_GRID) off += align_up(static_cast<size_t>(plan->n_wlayers) * 4 * Ng * Ng * sizeof(float2));
   a.work = off;   off += align_up(stack_bytes(plan, plan->batch_capacity));
   a.total = off;
   return a;
@@ -426,9 +428,8 @@ ArenaLayout arena_layout(const idg_plan* plan) {
 }  // namespace
 
 size_t idg_host_arena_bytes(const idg_plan* plan, int direction) {
-  (void)direction;
   if (!plan) return 0;
-  return arena_layout(plan).total;
+  return arena_layout(plan, direction).total;
 }
 
 namespace {
@@ -510,36 +511,30 @@ int idg_grid_host(const idg_plan* plan, const void* vis_host, const void* aterms
   int rc = ensure_device(plan, &d);
   if (rc != IDG_OK) return rc;
   ensure_row_runs(plan);
-  // Copy lane: A-terms and taper, then per batch the visibility rows it is the first to read; the grid
-  // (accumulated into) goes up after the first batch's rows, for the first adder.  The compute stream
-  // waits per batch, so uploads overlap the gridding of earlier batches.
+  // Copy lane: A-terms and taper, then per batch the visibility rows it is the first to read.  The compute
+  // stream waits per batch, so uploads overlap the gridding of earlier batches.
   CopyLane lane;
   IDG_CUDA(lane.init());
   IDG_CUDA(lane.order(stream, lane.s));                 // the arena may still be in use by earlier work
   IDG_CUDA(cudaMemcpyAsync(base + a.aterms, aterms_host, at_b, cudaMemcpyHostToDevice, lane.s));
   IDG_CUDA(cudaMemcpyAsync(base + a.taper, taper_host, L * L * sizeof(float), cudaMemcpyHostToDevice, lane.s));
-  cudaEvent_t grid_up = nullptr;
+  // The caller's grid (accumulated into) is NOT on the critical path: the subgrids are added into a zeroed
+  // device grid while the caller's grid goes up to a second buffer behind the visibilities, and the two are
+  // summed once at the end.
+  IDG_CUDA(cudaMemsetAsync(base + a.grid, 0, grid_b, stream));
   for (size_t i = 0; i < plan->batches.size(); ++i) {
     for (const auto& run : plan->rows_first[i])
       IDG_CUDA(cudaMemcpyAsync(base + a.vis + run.first * row_b, static_cast<const char*>(vis_host) + run.first * row_b,
                                (run.second - run.first) * row_b, cudaMemcpyHostToDevice, lane.s));
     IDG_CUDA(lane.order(lane.s, stream));
-    if (i == 0) {
-      IDG_CUDA(cudaMemcpyAsync(base + a.grid, grid_host, grid_b, cudaMemcpyHostToDevice, lane.s));
-      IDG_CUDA(lane.event(&grid_up));
-      IDG_CUDA(cudaEventRecord(grid_up, lane.s));
-    }
     rc = grid_batch(plan, d, i, base + a.vis, base + a.aterms, reinterpret_cast<const float*>(base + a.taper),
-                    base + a.grid, reinterpret_cast<float2*>(base + a.work), stream, [&]() -> int {
-                      if (i == 0) IDG_CUDA(cudaStreamWaitEvent(stream, grid_up, 0));
-                      return IDG_OK;
-                    });
+                    base + a.grid, reinterpret_cast<float2*>(base + a.work), stream, [] { return IDG_OK; });
     if (rc != IDG_OK) return rc;
   }
-  if (plan->batches.empty()) {
-    IDG_CUDA(cudaMemcpyAsync(base + a.grid, grid_host, grid_b, cudaMemcpyHostToDevice, lane.s));
-    IDG_CUDA(lane.order(lane.s, stream));
-  }
+  IDG_CUDA(cudaMemcpyAsync(base + a.grid_in, grid_host, grid_b, cudaMemcpyHostToDevice, lane.s));
+  IDG_CUDA(lane.order(lane.s, stream));
+  IDG_CUDA(launch_grid_add(reinterpret_cast<const float2*>(base + a.grid_in), reinterpret_cast<float2*>(base + a.grid),
+                           static_cast<int64_t>(grid_b / sizeof(float2)), stream));
   IDG_CUDA(cudaMemcpyAsync(grid_host, base + a.grid, grid_b, cudaMemcpyDeviceToHost, stream));
   IDG_CUDA(cudaStreamSynchronize(stream));
   IDG_CUDA(cudaStreamSynchronize(lane.s));
@@ -552,7 +547,7 @@ int idg_degrid_host(const idg_plan* plan, const void* grid_host, const void* ate
     set_error("idg_degrid_host: null argument");
     return IDG_EINVAL;
   }
-  const ArenaLayout a = arena_layout(plan);
+  const ArenaLayout a = arena_layout(plan, IDG_DEGRID);
   if (arena_bytes < a.total) { set_error("idg_degrid_host: arena too small (see idg_host_arena_bytes)"); return IDG_ENOMEM; }
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   char* base = static_cast<char*>(arena_dev);

@@ -53,6 +53,9 @@ cudaError_t launch_adder(const int32_t* meta, const DeviceCsr& csr, int64_t firs
                          int tiles_x, int tiles_y, const float2* subgrids, float2* grid,
                          cudaStream_t stream);
 
+// dst[i] += src[i] over n complex samples
+cudaError_t launch_grid_add(const float2* src, float2* dst, int64_t n, cudaStream_t stream);
+
 // step a6: splitter (gather).
 cudaError_t launch_splitter(const int32_t* meta, int64_t first, int64_t count, int L, int Ng,
                             const float2* grid, float2* subgrids, cudaStream_t stream);

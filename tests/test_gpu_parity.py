@@ -272,6 +272,10 @@ def test_host_buffer_calls(idg):
     idg.grid_host(plan, h_vis, h_at, h_tp, h_grid, arena)
     ref = orc.grid(par, sub, obs.uvw, obs.freqs, obs.vis, obs.baselines, obs.aterms, obs.taper)
     assert nerr(h_grid.numpy(), ref) <= TOL
+    # the grid is accumulated into: a second call on a non-zero grid adds the same again
+    before = h_grid.numpy().copy()
+    idg.grid_host(plan, h_vis, h_at, h_tp, h_grid, arena)
+    assert nerr(h_grid.numpy(), before.astype(np.complex128) + ref) <= TOL
     h_out = torch.zeros((cfg.n_rows, cfg.n_chan, 4), dtype=torch.complex64).pin_memory()
     G = torch.from_numpy(ref.astype(np.complex64)).pin_memory()
     idg.degrid_host(plan, G, h_at, h_tp, h_out, arena)
