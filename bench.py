@@ -414,13 +414,11 @@ def run_ours(args):
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
         dt, e2e_value = replicas_aggregate(dt, n_vis * n_e2e, world)
-        nb = lambda x: x.numel() * x.element_size()  # noqa: E731
-        # grid call: visibilities, A-terms, taper, grid up; degrid call: grid, A-terms, taper up, and the
-        # visibilities only when the planner left some uncovered (they must come back untouched)
-        covered = cnt.n_vis_planned == cfg.n_rows * cfg.n_chan
-        h2d = (nb(h_vis) + nb(h_at) + nb(h_tp) + nb(h_grid)) + (nb(h_at) + nb(h_tp) + nb(h_grid)) \
-            + (0 if covered else nb(h_vis))
-        d2h = nb(h_grid) + nb(h_out)
+        # what the two calls move over the bus, from the library (visibility rows and master-grid rows under a
+        # subgrid, A-terms, taper; the degrid call uploads visibilities only if the planner left some uncovered)
+        up_g, down_g = plan.host_traffic_bytes(idg.IDG_GRID)
+        up_d, down_d = plan.host_traffic_bytes(idg.IDG_DEGRID)
+        h2d, d2h = up_g + up_d, down_g + down_d
         e2e = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "steps": n_e2e, "ms_per_step": 1e3 * dt / n_e2e,
                "api": "idg_grid_host + idg_degrid_host (pinned host buffers; copies inside the calls, "

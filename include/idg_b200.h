@@ -129,12 +129,16 @@ IDG_API int  idg_degrid(const idg_plan* plan, const void* grid_dev, const void* 
 /* ---- the same two calls on HOST buffers (pinned memory recommended: pageable memory makes the
  * copies synchronous).  They copy the inputs to `arena_dev`, run the device path on `cuda_stream`,
  * copy the result back (grid_host is accumulated into: it is uploaded behind the visibilities and added
- * on the device after the subgrids) and synchronise before returning.  Copies run on a second stream and overlap compute batch by batch: a visibility row
+ * on the device after the subgrids) and synchronise before returning.  Only the master-grid rows under
+ * a subgrid are moved, in either direction: the rest of grid_host is neither read nor written.  Copies run on a second stream and overlap compute batch by batch: a visibility row
  * goes up just before the first batch that reads it and comes down right after the last batch
  * that writes it, so a plan with smaller batches (idg_params.max_batch_subgrids) overlaps more.
  * idg_degrid_host uploads vis_host only when the planner left visibilities uncovered (they come
  * back untouched).  arena_dev must hold idg_host_arena_bytes(plan, direction) bytes. */
 IDG_API size_t idg_host_arena_bytes(const idg_plan* plan, int direction);
+/* Bytes one idg_grid_host / idg_degrid_host call moves over the bus in each direction: the visibility rows
+ * and the master-grid rows that lie under a subgrid, the A-terms and the taper (nothing else is touched). */
+IDG_API int  idg_host_traffic_bytes(const idg_plan* plan, int direction, int64_t* h2d_bytes, int64_t* d2h_bytes);
 IDG_API int  idg_grid_host(const idg_plan* plan, const void* vis_host, const void* aterms_host,
                    const float* taper_host, void* grid_host, void* arena_dev, size_t arena_bytes,
                    void* cuda_stream);

@@ -23,7 +23,7 @@ STAGE_GRIDDER, STAGE_FFT = 0, 1
 # every symbol include/idg_b200.h declares
 SYMBOLS = (
     "idg_plan_create", "idg_plan_destroy", "idg_plan_counts", "idg_plan_export", "idg_workspace_bytes",
-    "idg_grid", "idg_grid_weighted", "idg_degrid", "idg_host_arena_bytes", "idg_grid_host", "idg_degrid_host",
+    "idg_grid", "idg_grid_weighted", "idg_degrid", "idg_host_arena_bytes", "idg_host_traffic_bytes", "idg_grid_host", "idg_degrid_host",
     "idg_grid_subgrids", "idg_degrid_subgrids", "idg_subgrid_fft", "idg_adder", "idg_splitter",
     "idg_closure_workspace_bytes", "idg_grid_to_image", "idg_image_to_grid",
     "idg_profile_enable", "idg_profile_read", "idg_set_kernel_variant", "idg_get_kernel_variant",
@@ -72,6 +72,8 @@ def load_library() -> ctypes.CDLL:
     lib.idg_workspace_bytes.restype = sz
     lib.idg_host_arena_bytes.argtypes = [vp, ctypes.c_int]
     lib.idg_host_arena_bytes.restype = sz
+    lib.idg_host_traffic_bytes.argtypes = [vp, ctypes.c_int, ctypes.POINTER(i64), ctypes.POINTER(i64)]
+    lib.idg_host_traffic_bytes.restype = ctypes.c_int
     lib.idg_grid.argtypes = [vp, vp, vp, vp, vp, vp, sz, vp]
     lib.idg_grid.restype = ctypes.c_int
     lib.idg_grid_weighted.argtypes = [vp, vp, vp, vp, vp, vp, vp, sz, vp]
@@ -205,6 +207,13 @@ class Plan:
 
     def host_arena_bytes(self, direction=IDG_GRID) -> int:
         return int(load_library().idg_host_arena_bytes(self._h, direction))
+
+    def host_traffic_bytes(self, direction=IDG_GRID):
+        """(host-to-device, device-to-host) bytes of one grid_host / degrid_host call."""
+        up, down = ctypes.c_int64(), ctypes.c_int64()
+        _check(load_library().idg_host_traffic_bytes(self._h, direction, ctypes.byref(up), ctypes.byref(down)),
+               "idg_host_traffic_bytes")
+        return int(up.value), int(down.value)
 
     def closure_workspace_bytes(self) -> int:
         return int(load_library().idg_closure_workspace_bytes(self._h))

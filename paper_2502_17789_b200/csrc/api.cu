@@ -464,6 +464,39 @@ void ensure_row_runs(const idg_plan* plan) {
   };
   runs(first, &plan->rows_first);
   runs(last, &plan->rows_last);
+  // master-grid rows under the subgrids of each w-layer: nothing outside them is read or written
+  plan->grid_rows.assign(plan->n_wlayers, {plan->par.grid_size, 0});
+  for (int64_t s = 0; s < plan->n_subgrids; ++s) {
+    const int32_t* m = &plan->sub[static_cast<size_t>(s) * 8];
+    auto& gr = plan->grid_rows[m[7] - plan->wl_min];
+    gr.first = std::min(gr.first, m[6]);
+    gr.second = std::max(gr.second, m[6] + plan->par.subgrid_size);
+  }
+  for (auto& gr : plan->grid_rows)
+    if (gr.second <= gr.first) gr = {0, 0};
+}
+
+// Copies the touched rows of every (layer, polarisation) plane of the master grid between host and device
+// (kind says which way); returns the bytes moved through `bytes` when it is not null.
+cudaError_t copy_grid_rows(const idg_plan* plan, void* dst, const void* src, cudaMemcpyKind kind, cudaStream_t stream,
+                           int64_t* bytes) {
+  const size_t Ng = plan->par.grid_size;
+  int64_t total = 0;
+  for (int32_t k = 0; k < plan->n_wlayers; ++k) {
+    const auto gr = plan->grid_rows[k];
+    const size_t n = static_cast<size_t>(gr.second - gr.first) * Ng * sizeof(float2);
+    if (n == 0) continue;
+    for (int p = 0; p < 4; ++p) {
+      const size_t off = ((static_cast<size_t>(k) * 4 + p) * Ng + gr.first) * Ng * sizeof(float2);
+      if (dst) {
+        cudaError_t e = cudaMemcpyAsync(static_cast<char*>(dst) + off, static_cast<const char*>(src) + off, n, kind, stream);
+        if (e != cudaSuccess) return e;
+      }
+      total += static_cast<int64_t>(n);
+    }
+  }
+  if (bytes) *bytes = total;
+  return cudaSuccess;
 }
 
 // a second stream and the events that order it against the caller's stream; all destroyed on return
@@ -491,6 +524,32 @@ struct CopyLane {
 };
 
 }  // namespace
+
+int idg_host_traffic_bytes(const idg_plan* plan, int direction, int64_t* h2d_bytes, int64_t* d2h_bytes) {
+  if (!plan || (direction != IDG_GRID && direction != IDG_DEGRID)) { set_error("idg_host_traffic_bytes: bad argument"); return IDG_EINVAL; }
+  ensure_row_runs(plan);
+  const idg_params& p = plan->par;
+  const int64_t L = p.subgrid_size;
+  const int64_t row_b = static_cast<int64_t>(p.n_chan) * 4 * sizeof(float2);
+  const int64_t at_b = static_cast<int64_t>(p.n_stations) * plan->n_intervals * L * L * 4 * sizeof(float2);
+  const int64_t tp_b = L * L * sizeof(float);
+  int64_t grid_rows_b = 0, vis_rows = 0;
+  copy_grid_rows(plan, nullptr, nullptr, cudaMemcpyHostToDevice, nullptr, &grid_rows_b);
+  for (const auto& runs : plan->rows_first)
+    for (const auto& run : runs) vis_rows += run.second - run.first;
+  const bool partial_rows = plan->n_vis_planned != static_cast<int64_t>(plan->n_rows) * p.n_chan;
+  int64_t up, down;
+  if (direction == IDG_GRID) {
+    up = vis_rows * row_b + at_b + tp_b + grid_rows_b;
+    down = grid_rows_b;
+  } else {
+    up = grid_rows_b + at_b + tp_b + (partial_rows ? static_cast<int64_t>(plan->n_rows) * row_b : 0);
+    down = vis_rows * row_b;
+  }
+  if (h2d_bytes) *h2d_bytes = up;
+  if (d2h_bytes) *d2h_bytes = down;
+  return IDG_OK;
+}
 
 int idg_grid_host(const idg_plan* plan, const void* vis_host, const void* aterms_host, const float* taper_host,
                   void* grid_host, void* arena_dev, size_t arena_bytes, void* cuda_stream) {
@@ -531,11 +590,13 @@ int idg_grid_host(const idg_plan* plan, const void* vis_host, const void* aterms
                     base + a.grid, reinterpret_cast<float2*>(base + a.work), stream, [] { return IDG_OK; });
     if (rc != IDG_OK) return rc;
   }
-  IDG_CUDA(cudaMemcpyAsync(base + a.grid_in, grid_host, grid_b, cudaMemcpyHostToDevice, lane.s));
+  // only the master-grid rows under the subgrids move: the rest of grid_host is already what it will be
+  IDG_CUDA(cudaMemsetAsync(base + a.grid_in, 0, grid_b, lane.s));
+  IDG_CUDA(copy_grid_rows(plan, base + a.grid_in, grid_host, cudaMemcpyHostToDevice, lane.s, nullptr));
   IDG_CUDA(lane.order(lane.s, stream));
   IDG_CUDA(launch_grid_add(reinterpret_cast<const float2*>(base + a.grid_in), reinterpret_cast<float2*>(base + a.grid),
                            static_cast<int64_t>(grid_b / sizeof(float2)), stream));
-  IDG_CUDA(cudaMemcpyAsync(grid_host, base + a.grid, grid_b, cudaMemcpyDeviceToHost, stream));
+  IDG_CUDA(copy_grid_rows(plan, grid_host, base + a.grid, cudaMemcpyDeviceToHost, stream, nullptr));
   IDG_CUDA(cudaStreamSynchronize(stream));
   IDG_CUDA(cudaStreamSynchronize(lane.s));
   return IDG_OK;
@@ -572,7 +633,8 @@ int idg_degrid_host(const idg_plan* plan, const void* grid_host, const void* ate
     IDG_CUDA(cudaMemcpyAsync(base + a.vis, vis_host, vis_b, cudaMemcpyHostToDevice, lane.s));
     IDG_CUDA(lane.order(lane.s, stream));
   }
-  IDG_CUDA(cudaMemcpyAsync(base + a.grid, grid_host, grid_b, cudaMemcpyHostToDevice, stream));
+  // the splitter reads the grid only under the subgrids: those rows go up, nothing else
+  IDG_CUDA(copy_grid_rows(plan, base + a.grid, grid_host, cudaMemcpyHostToDevice, stream, nullptr));
   IDG_CUDA(cudaMemcpyAsync(base + a.aterms, aterms_host, at_b, cudaMemcpyHostToDevice, stream));
   IDG_CUDA(cudaMemcpyAsync(base + a.taper, taper_host, L * L * sizeof(float), cudaMemcpyHostToDevice, stream));
   // per batch: predict, then download the rows it was the last to write while the next batch computes

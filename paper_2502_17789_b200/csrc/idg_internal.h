@@ -74,6 +74,8 @@ struct idg_plan {
   std::vector<idg::Batch> batches;
   // rows of the visibility table grouped by the first / last batch that touches them (host-buffer calls)
   mutable std::vector<std::vector<std::pair<int64_t, int64_t>>> rows_first, rows_last;
+  // per w-layer, the master-grid rows [first, last) under any subgrid: all the host-buffer calls move
+  mutable std::vector<std::pair<int32_t, int32_t>> grid_rows;
   mutable std::mutex mu;
   mutable idg::DeviceState* dev = nullptr;   // uploaded on first device call
 };

@@ -272,12 +272,26 @@ def test_host_buffer_calls(idg):
     idg.grid_host(plan, h_vis, h_at, h_tp, h_grid, arena)
     ref = orc.grid(par, sub, obs.uvw, obs.freqs, obs.vis, obs.baselines, obs.aterms, obs.taper)
     assert nerr(h_grid.numpy(), ref) <= TOL
-    # the grid is accumulated into: a second call on a non-zero grid adds the same again
+    # the grid is accumulated into: a second call on a non-zero grid adds the same again; rows of the grid
+    # under no subgrid are neither read nor written (only the touched rows cross the bus)
+    y_lo, y_hi = int(sub[:, 6].min()), int(sub[:, 6].max()) + cfg.subgrid_size
+    assert y_lo > 0 and y_hi < Ng
+    h_grid[:, :, :y_lo, :] = 3.0 - 2.0j
+    h_grid[:, :, y_hi:, :] = -1.0 + 5.0j
     before = h_grid.numpy().copy()
     idg.grid_host(plan, h_vis, h_at, h_tp, h_grid, arena)
-    assert nerr(h_grid.numpy(), before.astype(np.complex128) + ref) <= TOL
+    want = before.astype(np.complex128)
+    want[:, :, y_lo:y_hi, :] += ref[:, :, y_lo:y_hi, :]
+    assert nerr(h_grid.numpy(), want) <= TOL
+    assert np.array_equal(h_grid.numpy()[:, :, :y_lo, :], before[:, :, :y_lo, :])
+    assert np.array_equal(h_grid.numpy()[:, :, y_hi:, :], before[:, :, y_hi:, :])
+    up, down = plan.host_traffic_bytes(idg.IDG_GRID)
+    assert down == cnt.n_wlayers * 4 * (y_hi - y_lo) * Ng * 8 and up > down
     h_out = torch.zeros((cfg.n_rows, cfg.n_chan, 4), dtype=torch.complex64).pin_memory()
-    G = torch.from_numpy(ref.astype(np.complex64)).pin_memory()
+    Gn = ref.astype(np.complex64)
+    Gn[:, :, :y_lo, :] = np.nan                       # rows under no subgrid must not matter
+    Gn[:, :, y_hi:, :] = np.nan
+    G = torch.from_numpy(Gn).pin_memory()
     idg.degrid_host(plan, G, h_at, h_tp, h_out, arena)
     vref = orc.degrid(par, sub, obs.uvw, obs.freqs, ref.astype(np.complex64), obs.baselines, obs.aterms, obs.taper)
     assert nerr(h_out.numpy(), vref) <= TOL
