@@ -229,7 +229,7 @@ class ClockSampler:
         self.p = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.FIELDS}",
-                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                       "--format=csv,noheader,nounits", "-lms", "50"],
                                       stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
@@ -360,10 +360,12 @@ def run_ours(args):
             dist.barrier()
             torch.cuda.synchronize()
 
+    # clocks and throttle reasons are sampled from the warm-up steps on (nvidia-smi takes a moment to start and
+    # the timed region of the default run is under a second); the GPU runs the same kernels throughout
+    sampler = ClockSampler(torch.cuda.current_device()) if rank == 0 else None
     for _ in range(max(args.warmup, 3)):
         step()
     barrier()
-    sampler = ClockSampler(torch.cuda.current_device()) if rank == 0 else None
     idg.profile_read()
     idg.profile_enable(True)
     launches0 = idg.launch_count()
