@@ -114,9 +114,10 @@ def main():
           "with the padding as in the paper's Fig. 3 (`PAPER.md:299`); the fp32 columns follow it down to the "
           "single-precision floor (the paper's fp32 peak error is 43 uJy on 6.9 Jy = 6e-6, `:313`), where more "
           "padding buys nothing.  The SIMT gridder's floor is 3e-7-7e-7: its rounding errors are random and "
-          "average down over subgrids.  The tensor-core gridder's floor is 1.8e-6: the tensor core's fp32 "
-          "accumulation truncates, a bias that is coherent across subgrids (0.9e-6 with accumulator groups of 3 "
-          "chunks, 1.3e-6 with 6, 1.8e-6 with the default 12; DESIGN.md \"Tensor-core gridder\", Precision).")
+          "average down over subgrids.  The tensor-core gridder's floor is 0.8e-6-1.1e-6: the tensor core's fp32 "
+          "accumulation truncates, a bias that is coherent across subgrids (24 MMAs per accumulator with the fp16 "
+          "operands; the earlier split-tf32 operands, 48 MMAs, gave 1.8e-6; DESIGN.md \"Tensor-core gridder\", "
+          "Precision).")
 
 
 if __name__ == "__main__":
