@@ -10,7 +10,9 @@ Every function cites the passage of /root/reference/PAPER.md (arxiv 2502.17789) 
 §8(c)).  Pins: tests/test_oracle_pins.py checks this file against brute-force evaluation of
 the measurement equation (P1), point-source recovery (P2), the adjoint identity (P3), the
 closed-form gridding kernel (P4), prediction accuracy (P5), numpy.fft (P6), planner
-invariants (P7), adder/splitter adjointness (P8) and n' in extended precision (P9).
+invariants (P7), adder/splitter adjointness (P8), n' in extended precision (P9), the
+w >= 0 conjugation against the measurement equation's Hermitian symmetry (P11) and the
+power normalisation against an explicit Frobenius norm and its exact-correction case (P12).
 Parity unpinned: nothing.
 
 Conventions:
@@ -44,6 +46,10 @@ class OracleParams:
     n_chan: int
     aterm_period: int
     comfort: float = 0.75
+    # PAPER.md:178 (footnote 4): force w >= 0 by V(u,v,w) = V(-u,-v,-w)^dagger; reading R21 in DESIGN.md
+    positive_w: bool = False
+    # PAPER.md:257 (section 3.3): divide the subgrid by the Frobenius norm of M_p M_q^H; reading R22
+    power_norm: bool = False
 
     @property
     def image_size(self) -> float:
@@ -76,7 +82,11 @@ def plan(par: OracleParams, uvw_m: np.ndarray, freqs: np.ndarray, n_baselines: i
     dropped = 0
     bls = range(n_baselines) if baseline_subset is None else baseline_subset
     for b in bls:
-        rows = uvw_m[b * nT:(b + 1) * nT]
+        rows = np.asarray(uvw_m[b * nT:(b + 1) * nT], np.float64)
+        # PAPER.md:178 (fn 4): a row with w < 0 is used as the row (-u,-v,-w) of the swapped baseline
+        # (R21); its subgrids then lie in layers wl >= 0.  A subgrid never mixes the two kinds of row.
+        FLIP = (rows[:, 2] < 0.0) if par.positive_w else np.zeros(nT, bool)
+        rows = np.where(FLIP[:, None], -rows, rows)
         X = (rows[:, 0:1] * kappa[None, :]) * S          # [t, c]  exactly this fp64 order
         Y = (rows[:, 1:2] * kappa[None, :]) * S
         if par.w_step > 0:
@@ -103,7 +113,7 @@ def plan(par: OracleParams, uvw_m: np.ndarray, freqs: np.ndarray, n_baselines: i
                 n = 1
                 while t0 + n < tb:
                     t = t0 + n
-                    if WL[t, lo] != wl0 or WL[t, c1] != wl0:
+                    if WL[t, lo] != wl0 or WL[t, c1] != wl0 or FLIP[t] != FLIP[t0]:
                         break
                     nxmin = min(xmin, X[t, lo], X[t, c1]); nxmax = max(xmax, X[t, lo], X[t, c1])
                     nymin = min(ymin, Y[t, lo], Y[t, c1]); nymax = max(ymax, Y[t, lo], Y[t, c1])
@@ -157,11 +167,27 @@ def subgrid_centre(par: OracleParams, sub):
     return u0, v0, w0
 
 
+def subgrid_conjugated(par, sub, uvw_m):
+    """True when the subgrid's rows are used in their conjugated form (PAPER.md:178 fn 4, R21):
+    the plan asked for w >= 0 and the rows' w is negative (all rows of a subgrid agree, O1)."""
+    if not par.positive_w:
+        return False
+    b, t0 = int(sub[0]), int(sub[1])
+    return bool(uvw_m[b * par.n_times + t0][2] < 0.0)
+
+
+def dagger(V):
+    """V^dagger of row-major 2x2 matrices stored as [..., 4] = (XX, XY, YX, YY)."""
+    return np.conj(np.asarray(V)[..., [0, 2, 1, 3]])
+
+
 def _subgrid_relative_uvw(par, sub, uvw_m, freqs):
     b, t0, nt, c0, nc = (int(v) for v in sub[:5])
     kappa = np.asarray(freqs[c0:c0 + nc], np.float64) / C_LIGHT
     r0 = b * par.n_times + t0
     rows = np.asarray(uvw_m[r0:r0 + nt], np.float64)
+    if subgrid_conjugated(par, sub, uvw_m):
+        rows = -rows                                     # V(u,v,w) = V(-u,-v,-w)^dagger, PAPER.md:178
     u0, v0, w0 = subgrid_centre(par, sub)
     du = rows[:, 0:1] * kappa[None, :] - u0              # [nt, nc]
     dv = rows[:, 1:2] * kappa[None, :] - v0
@@ -176,9 +202,6 @@ def _phase(par, du, dv, dw):
             + dw[:, None, None] * n1[None, :, :])
 
 
-_KCHUNK = 96
-
-
 # ======================================================================================
 # O2  gridder: S[y,x] = sum_k V_k exp(+2 pi i phi)      (Eq. 10 :133-137; 2x2 per :253)
 # ======================================================================================
@@ -187,34 +210,60 @@ def gridder_subgrid(par, sub, uvw_m, freqs, vis):
     b, t0, nt, c0, nc = (int(v) for v in sub[:5])
     r0, du, dv, dw = _subgrid_relative_uvw(par, sub, uvw_m, freqs)
     V = np.asarray(vis[r0:r0 + nt, c0:c0 + nc, :], np.complex128).reshape(nt * nc, 4)
-    L = par.subgrid_size
-    S = np.zeros((L, L, 4), np.complex128)
-    for k0 in range(0, V.shape[0], _KCHUNK):
-        k1 = min(k0 + _KCHUNK, V.shape[0])
-        E = np.exp(2j * np.pi * _phase(par, du[k0:k1], dv[k0:k1], dw[k0:k1]))
-        S += np.einsum("kyx,kp->yxp", E, V[k0:k1])
-    return S
+    if subgrid_conjugated(par, sub, uvw_m):
+        V = dagger(V)
+    E = np.exp(2j * np.pi * _phase(par, du, dv, dw))     # one sum over k, as Eq. 10 is written
+    return np.einsum("kyx,kp->yxp", E, V)
 
 
 # ======================================================================================
 # O3 / O8  A-term sandwich and taper:  S' = T * M_p * S * M_q^H   (PAPER.md :156, :251-257; R5)
 # ======================================================================================
-def aterm_taper(S, Mp, Mq, taper):
-    """S [L,L,4] -> taper[y,x] * M_p[y,x] @ S[y,x] @ M_q[y,x]^H, per pixel (2x2 row-major)."""
+def aterm_taper(S, Mp, Mq, taper, power_norm=False):
+    """S [L,L,4] -> taper[y,x] * M_p[y,x] @ S[y,x] @ M_q[y,x]^H, per pixel (2x2 row-major).
+    power_norm (imaging only, R22): the result is divided by || M_p M_q^H ||_F per pixel."""
     L = S.shape[0]
     X = S.reshape(L, L, 2, 2)
     Mp = np.asarray(Mp, np.complex128)
     Mq = np.asarray(Mq, np.complex128)
     Y = np.einsum("yxab,yxbc,yxdc->yxad", Mp, X, np.conj(Mq), optimize=True)
-    return (np.asarray(taper, np.float64)[:, :, None, None] * Y).reshape(L, L, 4)
+    out = np.asarray(taper, np.float64)[:, :, None, None] * Y
+    if power_norm:
+        out = out * power_norm_factor(Mp, Mq)[:, :, None, None]
+    return out.reshape(L, L, 4)
 
 
-def subgrid_jones(par, sub, baselines, aterms):
-    """(M_p, M_q) maps of a subgrid: interval it = t0 div aterm_period (R6), stations of b."""
+def power_norm_factor(Mp, Mq):
+    """f[y,x] = 1 / || M_p[y,x] M_q[y,x]^H ||_F  ('normalising I-hat by the Frobenius norm of
+    the product A_1^-1 (A_2^-1)^dagger'; the maps given ARE the A^-1 of paper-style imaging, R5)."""
+    Pm = np.einsum("yxab,yxcb->yxac", np.asarray(Mp, np.complex128), np.conj(np.asarray(Mq, np.complex128)))
+    return 1.0 / np.sqrt((np.abs(Pm) ** 2).sum(axis=(2, 3)))
+
+
+def subgrid_jones(par, sub, baselines, aterms, uvw_m=None):
+    """(M_p, M_q) maps of a subgrid: interval it = t0 div aterm_period (R6), stations of b; the two swap
+    when the subgrid's rows are conjugated (PAPER.md:178 fn 4, R21; needs uvw_m to tell)."""
     b, t0 = int(sub[0]), int(sub[1])
     it = t0 // par.aterm_period
     p, q = int(baselines[b][0]), int(baselines[b][1])
+    if uvw_m is not None and subgrid_conjugated(par, sub, uvw_m):
+        p, q = q, p
     return aterms[p, it], aterms[q, it]
+
+
+def power_norm_average(par, subgrids, uvw_m, baselines, aterms):
+    """Weighted average over the subgrids of the normalisation factor, weights = visibilities per subgrid:
+    'the final image must then be corrected by the weighted average of this normalisation factor across all
+    subgrids' (PAPER.md:257, R22) -> float64 [L, L]."""
+    L = par.subgrid_size
+    num = np.zeros((L, L), np.float64)
+    den = 0.0
+    for sub in subgrids:
+        Mp, Mq = subgrid_jones(par, sub, baselines, aterms, uvw_m)
+        n = float(int(sub[2]) * int(sub[4]))
+        num += n * power_norm_factor(Mp, Mq)
+        den += n
+    return num / den
 
 
 # ======================================================================================
@@ -262,11 +311,10 @@ def degridder_subgrid(par, sub, uvw_m, freqs, Sp):
     """Sp [L,L,4] (after taper and A-term) -> complex128 [nt, nc, 4]."""
     b, t0, nt, c0, nc = (int(v) for v in sub[:5])
     _, du, dv, dw = _subgrid_relative_uvw(par, sub, uvw_m, freqs)
-    out = np.zeros((nt * nc, 4), np.complex128)
-    for k0 in range(0, out.shape[0], _KCHUNK):
-        k1 = min(k0 + _KCHUNK, out.shape[0])
-        E = np.exp(-2j * np.pi * _phase(par, du[k0:k1], dv[k0:k1], dw[k0:k1]))
-        out[k0:k1] = np.einsum("kyx,yxp->kp", E, Sp)
+    E = np.exp(-2j * np.pi * _phase(par, du, dv, dw))    # one sum over the pixels, as Eq. 13 is written
+    out = np.einsum("kyx,yxp->kp", E, Sp)
+    if subgrid_conjugated(par, sub, uvw_m):
+        out = dagger(out)                                # predicted V(-u,-v,-w) of (q,p) -> V(u,v,w) of (p,q)
     return out.reshape(nt, nc, 4)
 
 
@@ -276,8 +324,8 @@ def degridder_subgrid(par, sub, uvw_m, freqs, Sp):
 def grid_subgrid(par, sub, uvw_m, freqs, vis, baselines, aterms, taper):
     """Steps O2-O4 for one subgrid -> (S' after A-term+taper [L,L,4], Shat after FFT [L,L,4])."""
     S = gridder_subgrid(par, sub, uvw_m, freqs, vis)
-    Mp, Mq = subgrid_jones(par, sub, baselines, aterms)
-    Sp = aterm_taper(S, Mp, Mq, taper)
+    Mp, Mq = subgrid_jones(par, sub, baselines, aterms, uvw_m)
+    Sp = aterm_taper(S, Mp, Mq, taper, power_norm=par.power_norm)
     return Sp, subgrid_fft(Sp)
 
 
@@ -290,8 +338,8 @@ def degrid_subgrid(par, sub, uvw_m, freqs, grid, wl_min, baselines, aterms, tape
     L = par.subgrid_size
     patch = splitter(grid, sub, L, wl_min)
     S = subgrid_ifft(patch)
-    Mp, Mq = subgrid_jones(par, sub, baselines, aterms)
-    Sp = aterm_taper(S, Mp, Mq, taper)
+    Mp, Mq = subgrid_jones(par, sub, baselines, aterms, uvw_m)
+    Sp = aterm_taper(S, Mp, Mq, taper)                   # prediction is not power-normalised (R22)
     return Sp, degridder_subgrid(par, sub, uvw_m, freqs, Sp)
 
 

@@ -31,7 +31,7 @@ def _setup(cfg, seed=0, vis="hash", aterm="random"):
     return obs, par, sub, dropped, A, rng
 
 
-def _brute_force_image(cfg, par, obs, A, taper, sub_mask_rows=None):
+def _brute_force_image(cfg, par, obs, A, taper, sub_mask_rows=None, positive_w=False, power_norm=False):
     """taper[i] * sum_k M_p(l_i) V_k M_q(l_i)^H exp(+2 pi i (u_k l_i + v_k m_i + w_k n'_i)) at the
     L x L subgrid sample directions: the discrete imaging equation with A-terms, evaluated
     visibility by visibility straight from Eq. 1 / Eq. 2 of the paper (no subgrids, no FFT)."""
@@ -47,14 +47,26 @@ def _brute_force_image(cfg, par, obs, A, taper, sub_mask_rows=None):
         for t in range(cfg.n_times):
             r = b * cfg.n_times + t
             it = t // cfg.aterm_period
-            Mp = A[p, it].astype(np.complex128)
-            Mq = A[q, it].astype(np.complex128)
+            # PAPER.md:178 (fn 4): a sample with w < 0 may be used as the sample (-u,-v,-w) of the baseline
+            # (q, p), whose visibility is V^dagger -- the measurement equation's Hermitian symmetry
+            flip = positive_w and obs.uvw[r, 2] < 0
+            sgn = -1.0 if flip else 1.0
+            Mp = A[q if flip else p, it].astype(np.complex128)
+            Mq = A[p if flip else q, it].astype(np.complex128)
             acc = np.zeros((L, L, 2, 2), np.complex128)
             for c in range(cfg.n_chan):
-                u, v, w = obs.uvw[r] * kappa[c]
+                u, v, w = sgn * obs.uvw[r] * kappa[c]
                 ph = np.exp(1j * TWO_PI * (u * l + v * m + w * n1))
-                acc += ph[:, :, None, None] * obs.vis[r, c].astype(np.complex128).reshape(2, 2)[None, None]
-            out += Mp @ acc @ np.conj(np.swapaxes(Mq, -1, -2))
+                V = obs.vis[r, c].astype(np.complex128).reshape(2, 2)
+                if flip:
+                    V = V.conj().T
+                acc += ph[:, :, None, None] * V[None, None]
+            term = Mp @ acc @ np.conj(np.swapaxes(Mq, -1, -2))
+            if power_norm:
+                # divide by the Frobenius norm of the product of the two maps, per pixel
+                prod = Mp @ np.conj(np.swapaxes(Mq, -1, -2))
+                term = term / np.linalg.norm(prod, ord="fro", axis=(-2, -1))[:, :, None, None]
+            out += term
     return taper[:, :, None, None] * out
 
 
@@ -204,7 +216,13 @@ def _check_plan_invariants(cfg, obs, par, sub, dropped):
         assert 0 <= x0 and 0 <= y0 and x0 + L <= Ng and y0 + L <= Ng             # box inside grid
         r0 = b * cfg.n_times + t0
         cover[r0:r0 + nt, c0:c0 + nc] += 1
-        uvw = obs.uvw[r0:r0 + nt, None, :] * kappa[None, c0:c0 + nc, None]
+        rows = obs.uvw[r0:r0 + nt]
+        if par.positive_w:
+            neg = rows[:, 2] < 0
+            assert neg.all() or not neg.any(), "a subgrid mixes conjugated and plain rows"
+            rows = np.where(neg[:, None], -rows, rows)                            # fn 4: (u,v,w) -> -(u,v,w)
+            assert wl >= 0, "positive_w must leave no negative w-layer"
+        uvw = rows[:, None, :] * kappa[None, c0:c0 + nc, None]
         X, Y = uvw[..., 0] * S, uvw[..., 1] * S
         cx, cy = x0 + L // 2 - Ng // 2, y0 + L // 2 - Ng // 2
         # ALL members (not only the corners) within the usable span (R8)
@@ -268,7 +286,7 @@ def test_p8_adder_splitter():
 
 def test_p9_nprime_extended_precision():
     """P9: n' = sqrt(1-l^2-m^2) - 1 in the cancellation-free form, against 50-digit mpmath."""
-    mp = pytest.importorskip("mpmath")
+    import mpmath as mp
     mp.mp.dps = 50
     for l, m in [(1e-9, 0.0), (3e-5, -2e-5), (1e-3, 1e-3), (0.05, -0.07), (0.3, 0.4), (0.0, 0.0)]:
         ref = mp.sqrt(1 - mp.mpf(l) ** 2 - mp.mpf(m) ** 2) - 1
@@ -293,3 +311,167 @@ def test_subgrid_centre_and_phase_signs():
     ref = np.zeros_like(G)
     ref[0, :, py, px] = V.reshape(4)
     assert np.abs(G - ref).max() < 1e-12
+
+
+# ---------------------------------------------------------------------------------------------
+# P11  w >= 0 by conjugation (footnote 4; R21)
+# ---------------------------------------------------------------------------------------------
+def _dagger_image(img):
+    return np.conj(np.swapaxes(img, -1, -2))
+
+
+def test_p11_positive_w_brute_force_and_symmetry():
+    """With positive_w the closure image equals the direct transform of the conjugated samples
+    ((-u,-v,-w), baseline (q,p), V^dagger for every row with w < 0), all layers are >= 0 and fewer than with
+    signed layers, and the Hermitian part of the image -- all a Hermitian sky can populate -- is unchanged."""
+    cfg = tiny_config(w_step=3.0, ha_mid_deg=25.0)
+    obs, par, sub, dropped, A, rng = _setup(cfg, seed=4)
+    assert (obs.uvw[:, 2] < 0).any() and (obs.uvw[:, 2] > 0).any(), "need both signs of w"
+    par_c = dataclasses.replace(par, positive_w=True)
+    sub_c, dropped_c = orc.plan(par_c, obs.uvw, obs.freqs, cfg.n_baselines)
+    assert dropped_c == 0 and sub_c[:, 7].min() >= 0
+    assert orc.layer_range(sub_c)[1] < orc.layer_range(sub)[1], "fewer w-layers of master grid are needed"
+    _check_plan_invariants(cfg, obs, par_c, sub_c, dropped_c)
+    taper = rng.uniform(0.2, 1.0, (cfg.subgrid_size, cfg.subgrid_size))
+    L, Ng = cfg.subgrid_size, cfg.grid_size
+    j = Ng // 2 + (np.arange(L) - L // 2) * (Ng // L)
+    G_c = orc.grid(par_c, sub_c, obs.uvw, obs.freqs, obs.vis, obs.baselines, A, taper)
+    wl_min_c, _ = orc.layer_range(sub_c)
+    img_c = orc.image_at_pixels(par_c, G_c, wl_min_c, j, j).reshape(L, L, 2, 2)
+    ref_c = _brute_force_image(cfg, par_c, obs, A, taper, positive_w=True)
+    assert np.abs(img_c - ref_c).max() / np.abs(ref_c).max() < 1e-12
+    # Hermitian part: the same image as without the option
+    G = orc.grid(par, sub, obs.uvw, obs.freqs, obs.vis, obs.baselines, A, taper)
+    wl_min, _ = orc.layer_range(sub)
+    img = orc.image_at_pixels(par, G, wl_min, j, j).reshape(L, L, 2, 2)
+    h, h_c = img + _dagger_image(img), img_c + _dagger_image(img_c)
+    assert np.abs(h - h_c).max() / np.abs(h).max() < 1e-12
+    assert np.abs(img - img_c).max() / np.abs(img).max() > 1e-3, "the option must change something"
+
+
+def test_p11_positive_w_prediction_is_the_real_adjoint():
+    """The conjugation V -> V^dagger is conjugate-linear, so with positive_w the pair (degrid(.;M), grid(.;M^H))
+    is adjoint for the REAL inner product Re<a,b> (which is what an imaging major cycle minimises), and the
+    imaginary parts of the two sides are opposite on the conjugated rows only.  Pins O6-O9 with the option."""
+    cfg = tiny_config(w_step=3.0, ha_mid_deg=25.0)
+    obs, par, sub, dropped, A, rng = _setup(cfg, seed=6)
+    par_c = dataclasses.replace(par, positive_w=True)
+    sub_c, _ = orc.plan(par_c, obs.uvw, obs.freqs, cfg.n_baselines)
+    taper = synth.taper_subgrid(cfg).astype(np.float64)
+    wl_min, W = orc.layer_range(sub_c)
+    Ng = cfg.grid_size
+    G = rng.standard_normal((W, 4, Ng, Ng)) + 1j * rng.standard_normal((W, 4, Ng, Ng))
+    V = obs.vis.astype(np.complex128)
+    AH = np.conj(np.swapaxes(A, -1, -2))
+    pred = orc.degrid(par_c, sub_c, obs.uvw, obs.freqs, G, obs.baselines, A, taper)
+    lhs = inner(pred, V)
+    rhs = inner(G, orc.grid(par_c, sub_c, obs.uvw, obs.freqs, V, obs.baselines, AH, taper))
+    assert abs(lhs.real - rhs.real) / abs(lhs) < 1e-12, (lhs, rhs)
+    # row by row: plain rows obey the complex identity, conjugated rows its complex conjugate
+    neg = np.repeat(obs.uvw[:, 2] < 0, cfg.n_chan).reshape(cfg.n_rows, cfg.n_chan)
+    Vp, Vn = np.where(neg[..., None], 0, V), np.where(neg[..., None], V, 0)
+    for Vs, conj in ((Vp, False), (Vn, True)):
+        a = inner(pred, Vs)
+        b = inner(G, orc.grid(par_c, sub_c, obs.uvw, obs.freqs, Vs, obs.baselines, AH, taper))
+        assert abs(a - (np.conj(b) if conj else b)) / abs(a) < 1e-12
+
+
+def test_p11_positive_w_predicts_a_hermitian_sky():
+    """Prediction with positive_w from a physical (Hermitian-brightness) point source equals Eq. 1 evaluated
+    directly, like P5, on every row -- conjugated or not -- to the taper-limited tolerance."""
+    L, P, tol = 32, 12, 1e-7
+    cfg = tiny_config(subgrid_size=L, padding=P, w_step=3.0, ha_mid_deg=25.0)
+    obs, par, sub, dropped, A, rng = _setup(cfg, aterm="identity", vis=None)
+    par_c = dataclasses.replace(par, positive_w=True)
+    sub_c, _ = orc.plan(par_c, obs.uvw, obs.freqs, cfg.n_baselines)
+    Ng, S = cfg.grid_size, cfg.image_size
+    jy, jx = Ng // 2 - 41, Ng // 2 + 30
+    I, Q, U, Vs = 2.0, 0.3, -0.4, 0.25                      # Stokes -> Hermitian brightness matrix
+    B = np.array([I + Q, U + 1j * Vs, U - 1j * Vs, I - Q])
+    t1 = synth.taper_full_1d(Ng, P)
+    model = np.zeros((4, Ng, Ng), np.complex128)
+    model[:, jy, jx] = B / (t1[jy] * t1[jx])
+    wl_min, W = orc.layer_range(sub_c)
+    G = orc.model_to_grid(par_c, model, wl_min, W)
+    taper = synth.taper_subgrid(cfg).astype(np.float64)
+    V = orc.degrid(par_c, sub_c, obs.uvw, obs.freqs, G, obs.baselines, A, taper)
+    l0, m0 = (jx - Ng // 2) * S / Ng, (jy - Ng // 2) * S / Ng
+    n0 = np.sqrt(1 - l0 * l0 - m0 * m0) - 1
+    uvw = obs.uvw[:, None, :] * (obs.freqs / 299792458.0)[None, :, None]
+    ph = np.exp(-1j * TWO_PI * (uvw[..., 0] * l0 + uvw[..., 1] * m0 + uvw[..., 2] * n0))
+    ref = ph[..., None] * B[None, None, :]
+    assert np.abs(V - ref).max() / I < tol
+
+
+# ---------------------------------------------------------------------------------------------
+# P12  power normalisation by the Frobenius norm (PAPER.md:257, section 3.3; DESIGN.md R22)
+# ---------------------------------------------------------------------------------------------
+def test_p12_power_norm_brute_force():
+    """With power_norm every visibility's contribution to the image is divided, per pixel, by the Frobenius norm
+    of M_p M_q^H of its baseline and interval (numpy.linalg.norm on the explicit product)."""
+    cfg = tiny_config()
+    obs, par, sub, dropped, A, rng = _setup(cfg, seed=9)
+    par_n = dataclasses.replace(par, power_norm=True)
+    taper = rng.uniform(0.2, 1.0, (cfg.subgrid_size, cfg.subgrid_size))
+    G = orc.grid(par_n, sub, obs.uvw, obs.freqs, obs.vis, obs.baselines, A, taper)
+    wl_min, _ = orc.layer_range(sub)
+    L, Ng = cfg.subgrid_size, cfg.grid_size
+    j = Ng // 2 + (np.arange(L) - L // 2) * (Ng // L)
+    img = orc.image_at_pixels(par_n, G, wl_min, j, j).reshape(L, L, 2, 2)
+    ref = _brute_force_image(cfg, par_n, obs, A, taper, power_norm=True)
+    assert np.abs(img - ref).max() / np.abs(ref).max() < 1e-12
+    # the factor itself: sqrt of the sum of the squared singular values of the product
+    Mp, Mq = A[1, 0].astype(np.complex128), A[4, 0].astype(np.complex128)
+    sv = np.linalg.svd(Mp @ np.conj(np.swapaxes(Mq, -1, -2)), compute_uv=False)
+    assert np.abs(orc.power_norm_factor(Mp, Mq) * np.sqrt((sv ** 2).sum(-1)) - 1).max() < 1e-13
+
+
+def test_p12_power_norm_correction_is_exact_for_a_shared_aterm():
+    """'The final image must then be corrected by the weighted average of this normalisation factor across all
+    subgrids': when every station and interval shares one A-term map the average IS the factor,
+    so the corrected image equals the un-normalised one exactly; with different maps the weights are the
+    subgrids' visibility counts."""
+    cfg = tiny_config()
+    obs, par, sub, dropped, A, rng = _setup(cfg, seed=10)
+    A_shared = np.broadcast_to(A[0:1, 0:1], A.shape).copy()
+    par_n = dataclasses.replace(par, power_norm=True)
+    taper = synth.taper_subgrid(cfg).astype(np.float64)
+    L, Ng = cfg.subgrid_size, cfg.grid_size
+    j = Ng // 2 + (np.arange(L) - L // 2) * (Ng // L)
+    wl_min, _ = orc.layer_range(sub)
+    img = orc.image_at_pixels(par, orc.grid(par, sub, obs.uvw, obs.freqs, obs.vis, obs.baselines, A_shared, taper),
+                              wl_min, j, j)
+    img_n = orc.image_at_pixels(par_n, orc.grid(par_n, sub, obs.uvw, obs.freqs, obs.vis, obs.baselines, A_shared, taper),
+                                wl_min, j, j)
+    avg = orc.power_norm_average(par_n, sub, obs.uvw, obs.baselines, A_shared)
+    assert np.abs(img_n / avg[:, :, None] - img).max() / np.abs(img).max() < 1e-12
+    # general maps: the average weighs each subgrid's factor by its visibility count
+    avg2 = orc.power_norm_average(par_n, sub, obs.uvw, obs.baselines, A)
+    num, den = np.zeros((L, L)), 0
+    for s in sub:
+        p, q = obs.baselines[s[0]]
+        it = s[1] // cfg.aterm_period
+        prod = A[p, it].astype(np.complex128) @ np.conj(np.swapaxes(A[q, it].astype(np.complex128), -1, -2))
+        num += int(s[2]) * int(s[4]) / np.linalg.norm(prod, ord="fro", axis=(-2, -1))
+        den += int(s[2]) * int(s[4])
+    assert den == cfg.n_vis and np.abs(avg2 - num / den).max() < 1e-13
+
+
+def test_p12_power_norm_breaks_the_adjoint():
+    """R16/R22: the normalisation is applied in imaging only, so grid(.; M^H) with power_norm is no longer the
+    adjoint of degrid(.; M) -- the documented defect, asserted so that nobody 'fixes' one side silently."""
+    cfg = tiny_config()
+    obs, par, sub, dropped, A, rng = _setup(cfg, seed=12)
+    par_n = dataclasses.replace(par, power_norm=True)
+    taper = synth.taper_subgrid(cfg).astype(np.float64)
+    wl_min, W = orc.layer_range(sub)
+    Ng = cfg.grid_size
+    G = rng.standard_normal((W, 4, Ng, Ng)) + 1j * rng.standard_normal((W, 4, Ng, Ng))
+    V = obs.vis.astype(np.complex128)
+    AH = np.conj(np.swapaxes(A, -1, -2))
+    pred_n = orc.degrid(par_n, sub, obs.uvw, obs.freqs, G, obs.baselines, A, taper)
+    pred = orc.degrid(par, sub, obs.uvw, obs.freqs, G, obs.baselines, A, taper)
+    assert np.array_equal(pred_n, pred), "prediction must not be normalised"
+    lhs = inner(pred_n, V)
+    rhs = inner(G, orc.grid(par_n, sub, obs.uvw, obs.freqs, V, obs.baselines, AH, taper))
+    assert abs(lhs - rhs) / abs(lhs) > 1e-2
