@@ -307,6 +307,95 @@ def kernel_rooflines(cfg, sub, n_wlayers, prof_ms, prof_n, steps, peaks, sm_mhz_
     return out, peak_tflops, flop, alg_bytes
 
 
+OPERANDS = ("direct sums on tcgen05: gridder fp16 head + fp16 remainder of (cos, sin) and of the visibilities (one "
+            "power-of-two scale per segment), degridder tf32 head + tf32 remainder; fp32 accumulation in tensor memory, "
+            "drained into fp32 registers every 12 chunks; phase, sin/cos, A-term sandwich, FFT in fp32, adder sums in "
+            "fp64; sparsely filled subgrids take the all-fp32 SIMT kernels (kernel choice per subgrid)")
+
+
+def device_leg(idg, torch, cfg, plan, sub, cnt, d_vis, d_at, d_tp, steps, warmup, stream, barrier, peaks,
+               sampler_index=None, prediction_only=False):
+    """Times `steps` passes of the hot path on resident inputs with CUDA events on the launching stream, after
+    `warmup` untimed passes.  Returns a dict of whole-step, per-direction and per-kernel figures."""
+    Ng = cfg.grid_size
+    d_grid = torch.zeros((cnt.n_wlayers, 4, Ng, Ng), dtype=torch.complex64, device=d_vis.device)
+    d_out = torch.zeros_like(d_vis)
+    ws = torch.empty(max(plan.workspace_bytes(idg.IDG_GRID), plan.workspace_bytes(idg.IDG_DEGRID)),
+                     dtype=torch.uint8, device=d_vis.device)
+    if prediction_only:                                   # config 5: the grid is an input, made once
+        idg.grid(plan, d_vis, d_at, d_tp, d_grid, ws, stream)
+    # clocks and throttle reasons are sampled from the warm-up steps on (nvidia-smi takes a moment to start and
+    # the timed region of the default run is under a second); the GPU runs the same kernels throughout
+    sampler = ClockSampler(sampler_index) if sampler_index is not None else None
+
+    def one(k=None, ev=None):
+        if not prediction_only:
+            idg.grid(plan, d_vis, d_at, d_tp, d_grid, ws, stream)
+        if ev is not None:
+            ev[2 * k + 1].record(stream)
+        idg.degrid(plan, d_grid, d_at, d_tp, d_out, ws, stream)
+        if ev is not None:
+            ev[2 * k + 2].record(stream)
+
+    for _ in range(warmup):
+        one()
+    barrier()
+    idg.profile_read()
+    idg.profile_enable(True)
+    launches0 = idg.launch_count()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * steps + 1)]
+    ev[0].record(stream)
+    for k in range(steps):
+        one(k, ev)
+    barrier()
+    launches = idg.launch_count() - launches0
+    idg.profile_enable(False)
+    prof = idg.profile_read()
+    clocks = sampler.stop() if sampler else None
+    total_ms = ev[0].elapsed_time(ev[-1])
+    grid_ms = sum(ev[2 * k].elapsed_time(ev[2 * k + 1]) for k in range(steps)) / steps
+    degrid_ms = sum(ev[2 * k + 1].elapsed_time(ev[2 * k + 2]) for k in range(steps)) / steps
+    sm_obs = clocks["sm_mhz"] if clocks else None
+    prof_ms = {k: v[0] for k, v in prof.items()}
+    prof_n = {k: v[1] for k, v in prof.items()}
+    kr, peak_tflops, _, _ = kernel_rooflines(cfg, sub, cnt.n_wlayers, prof_ms, prof_n, steps, peaks, sm_obs)
+    n_vis = cnt.n_vis_planned
+    out = {"total_ms": total_ms, "ms_per_step": total_ms / steps, "degrid_ms": degrid_ms,
+           "degrid_vis_per_s": n_vis / (degrid_ms / 1e3), "kernels": kr, "clocks": clocks, "launches": int(launches),
+           "peak_tflops": peak_tflops, "n_subgrids": int(cnt.n_subgrids), "n_vis": int(n_vis),
+           "n_wlayers": int(cnt.n_wlayers)}
+    if not prediction_only:
+        out.update(grid_ms=grid_ms, grid_vis_per_s=n_vis / (grid_ms / 1e3))
+    del d_grid, d_out, ws
+    return out
+
+
+def other_config(idg, torch, config_id, dev, stream, barrier, peaks, sampler_index):
+    """One warm-up and two timed steps of another BASELINE.json config (3, 4: grid + degrid; 5: prediction only, from
+    the grid of one imaging pass), visibilities by the counter-based hash recipe generated on the device (the
+    values do not affect timing).  The headline `value`, `config` and `roofline` stay config 2's."""
+    cfg = synth.get_config(config_id)
+    obs = synth.make_observation(cfg, vis=None)
+    plan = idg.plan_from_config(cfg, obs.uvw, obs.freqs, obs.baselines)
+    sub = plan.export()
+    cnt = plan.counts()
+    d_vis = synth.hash_visibilities_torch(cfg.n_rows, cfg.n_chan, cfg.seed, dev)
+    d_at = torch.from_numpy(obs.aterms).to(dev)
+    d_tp = torch.from_numpy(obs.taper).to(dev)
+    r = device_leg(idg, torch, cfg, plan, sub, cnt, d_vis, d_at, d_tp, 2, 1, stream, barrier, peaks, sampler_index,
+                   prediction_only=(config_id == 5))
+    del d_vis, d_at, d_tp, plan
+    torch.cuda.empty_cache()
+    keep = {k: r[k] for k in ("ms_per_step", "grid_ms", "degrid_ms", "grid_vis_per_s", "degrid_vis_per_s", "n_subgrids",
+                              "n_vis", "n_wlayers", "clocks") if k in r}
+    keep["workload"] = workload_config(cfg)["workload"]
+    keep["steps"], keep["warmup"] = 2, 1
+    keep["kernels"] = {k: {"ms_per_step": v["ms_per_step"], "frac": v["frac"], "bound": v["bound"],
+                           **({"pairs_per_clk_per_sm": v["pairs_per_clk_per_sm"]} if "pairs_per_clk_per_sm" in v else {})}
+                       for k, v in r["kernels"].items()}
+    return keep
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -341,18 +430,13 @@ def run_ours(args):
     sub = plan.export()
     cnt = plan.counts()
     Ng = cfg.grid_size
-    d_vis = synth.source_visibilities_torch(obs.uvw, obs.freqs, obs.sources, dev)
+    if cfg.config_id in (3, 4, 5):
+        d_vis = synth.hash_visibilities_torch(cfg.n_rows, cfg.n_chan, cfg.seed, dev)
+    else:
+        d_vis = synth.source_visibilities_torch(obs.uvw, obs.freqs, obs.sources, dev)
     d_at = torch.from_numpy(obs.aterms).to(dev)
     d_tp = torch.from_numpy(obs.taper).to(dev)
-    d_grid = torch.zeros((cnt.n_wlayers, 4, Ng, Ng), dtype=torch.complex64, device=dev)
-    d_out = torch.zeros_like(d_vis)
-    ws = torch.empty(max(plan.workspace_bytes(idg.IDG_GRID), plan.workspace_bytes(idg.IDG_DEGRID)),
-                     dtype=torch.uint8, device=dev)
     stream = torch.cuda.current_stream()
-
-    def step():
-        idg.grid(plan, d_vis, d_at, d_tp, d_grid, ws, stream)
-        idg.degrid(plan, d_grid, d_at, d_tp, d_out, ws, stream)
 
     def barrier():
         torch.cuda.synchronize()
@@ -360,97 +444,89 @@ def run_ours(args):
             dist.barrier()
             torch.cuda.synchronize()
 
-    # clocks and throttle reasons are sampled from the warm-up steps on (nvidia-smi takes a moment to start and
-    # the timed region of the default run is under a second); the GPU runs the same kernels throughout
-    sampler = ClockSampler(torch.cuda.current_device()) if rank == 0 else None
-    for _ in range(max(args.warmup, 3)):
-        step()
-    barrier()
-    idg.profile_read()
-    idg.profile_enable(True)
-    launches0 = idg.launch_count()
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps + 1)]
-    ev[0].record(stream)
-    for k in range(args.steps):
-        idg.grid(plan, d_vis, d_at, d_tp, d_grid, ws, stream)
-        ev[2 * k + 1].record(stream)
-        idg.degrid(plan, d_grid, d_at, d_tp, d_out, ws, stream)
-        ev[2 * k + 2].record(stream)
-    barrier()
-    launches = idg.launch_count() - launches0
-    idg.profile_enable(False)
-    prof = idg.profile_read()
-    clocks = sampler.stop() if sampler else None
-    total_ms = ev[0].elapsed_time(ev[-1])
-    grid_ms = sum(ev[2 * k].elapsed_time(ev[2 * k + 1]) for k in range(args.steps)) / args.steps
-    degrid_ms = sum(ev[2 * k + 1].elapsed_time(ev[2 * k + 2]) for k in range(args.steps)) / args.steps
+    warmup = max(args.warmup, 3)
+    prediction_only = cfg.config_id == 5
+    leg = device_leg(idg, torch, cfg, plan, sub, cnt, d_vis, d_at, d_tp, args.steps, warmup, stream, barrier, peaks,
+                     torch.cuda.current_device() if rank == 0 else None, prediction_only)
     n_vis = cnt.n_vis_planned
-    total_s, value = replicas_aggregate(total_ms / 1e3, n_vis * args.steps, world)
-    total_ms = total_s * 1e3
-    ms_per_step = total_ms / args.steps
+    total_s, value = replicas_aggregate(leg["total_ms"] / 1e3, n_vis * args.steps, world)
+    ms_per_step = total_s * 1e3 / args.steps
 
     # end to end through the host-buffer C-ABI calls: pinned host -> device -> pinned host, every step
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not prediction_only:
         h_vis = d_vis.cpu().pin_memory()
         h_at = torch.from_numpy(obs.aterms).pin_memory()
         h_tp = torch.from_numpy(obs.taper).pin_memory()
         h_grid = torch.zeros((cnt.n_wlayers, 4, Ng, Ng), dtype=torch.complex64).pin_memory()
         h_out = torch.zeros((cfg.n_rows, cfg.n_chan, 4), dtype=torch.complex64).pin_memory()
-        del d_out, d_grid, ws
-        torch.cuda.empty_cache()
-        # the host-buffer calls pipeline copies against compute batch by batch: smaller batches overlap more
-        # (the device-resident leg above keeps the library's default batch, which is ~1 % faster on the device)
+        # the host-buffer calls pipeline copies against compute batch by batch: smaller batches overlap more.
+        # The device-resident headline keeps the library's default batch; the SAME plan the end-to-end leg uses is
+        # also timed device-resident below, so the two legs can be compared on one configuration of the library.
+        e2e_plan, same_plan_ms = plan, leg["ms_per_step"]
         if args.e2e_batch and not args.max_batch:
-            plan = idg.plan_from_config(cfg, obs.uvw, obs.freqs, obs.baselines, max_batch_subgrids=args.e2e_batch)
-        arena = torch.empty(max(plan.host_arena_bytes(idg.IDG_GRID), plan.host_arena_bytes(idg.IDG_DEGRID)),
+            e2e_plan = idg.plan_from_config(cfg, obs.uvw, obs.freqs, obs.baselines, max_batch_subgrids=args.e2e_batch)
+            same = device_leg(idg, torch, cfg, e2e_plan, sub, cnt, d_vis, d_at, d_tp, args.steps, 1, stream, barrier, peaks)
+            same_plan_ms = same["ms_per_step"]
+        torch.cuda.empty_cache()
+        arena = torch.empty(max(e2e_plan.host_arena_bytes(idg.IDG_GRID), e2e_plan.host_arena_bytes(idg.IDG_DEGRID)),
                             dtype=torch.uint8, device=dev)
-        n_e2e = max(1, min(args.steps, 3))
-        idg.grid_host(plan, h_vis, h_at, h_tp, h_grid, arena, stream)        # warm-up
-        idg.degrid_host(plan, h_grid, h_at, h_tp, h_out, arena, stream)
+        n_e2e = args.steps
+        idg.grid_host(e2e_plan, h_vis, h_at, h_tp, h_grid, arena, stream)        # warm-up
+        idg.degrid_host(e2e_plan, h_grid, h_at, h_tp, h_out, arena, stream)
         barrier()
         t0 = time.perf_counter()
         for _ in range(n_e2e):
-            idg.grid_host(plan, h_vis, h_at, h_tp, h_grid, arena, stream)
-            idg.degrid_host(plan, h_grid, h_at, h_tp, h_out, arena, stream)
+            idg.grid_host(e2e_plan, h_vis, h_at, h_tp, h_grid, arena, stream)
+            idg.degrid_host(e2e_plan, h_grid, h_at, h_tp, h_out, arena, stream)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
         dt, e2e_value = replicas_aggregate(dt, n_vis * n_e2e, world)
         # what the two calls move over the bus, from the library (visibility rows and master-grid rows under a
         # subgrid, A-terms, taper; the degrid call uploads visibilities only if the planner left some uncovered)
-        up_g, down_g = plan.host_traffic_bytes(idg.IDG_GRID)
-        up_d, down_d = plan.host_traffic_bytes(idg.IDG_DEGRID)
+        up_g, down_g = e2e_plan.host_traffic_bytes(idg.IDG_GRID)
+        up_d, down_d = e2e_plan.host_traffic_bytes(idg.IDG_DEGRID)
         h2d, d2h = up_g + up_d, down_g + down_d
         e2e = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": d2h, "steps": n_e2e, "ms_per_step": 1e3 * dt / n_e2e,
                "api": "idg_grid_host + idg_degrid_host (pinned host buffers; copies inside the calls, "
                       "overlapped with compute per batch on a second stream)",
-               "max_batch_subgrids": int(args.max_batch or args.e2e_batch)}
+               "max_batch_subgrids": int(args.max_batch or args.e2e_batch),
+               "device_resident_ms_per_step_same_plan": same_plan_ms}
+        del arena, h_vis, h_grid, h_out
+    del d_vis, d_at, d_tp
+    torch.cuda.empty_cache()
+
+    # the other single-GPU workloads of BASELINE.json, briefly (rank 0 of a 1-GPU run only)
+    others = None
+    if rank == 0 and world == 1 and cfg.config_id == 2 and not args.no_other_configs:
+        others = {}
+        for c in (3, 4, 5):
+            others[str(c)] = other_config(idg, torch, c, dev, stream, barrier, peaks, torch.cuda.current_device())
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return 0
-    sm_obs = clocks["sm_mhz"] if clocks else None
-    prof_ms = {k: v[0] for k, v in prof.items()}
-    prof_n = {k: v[1] for k, v in prof.items()}
-    kr, peak_tflops, flop, alg_bytes = kernel_rooflines(cfg, sub, cnt.n_wlayers, prof_ms, prof_n, args.steps, peaks,
-                                                        sm_obs)
-    dom = max(("gridder", "degridder"), key=lambda k: kr[k]["ms_per_step"])
-    roofline = {"kernel": dom, "bound": "alu", "achieved": kr[dom]["tflops"], "peak": peak_tflops,
+    kr, clocks = leg["kernels"], leg["clocks"]
+    cands = [k for k in ("gridder", "degridder") if k in kr]
+    dom = max(cands, key=lambda k: kr[k]["ms_per_step"])
+    roofline = {"kernel": dom, "bound": "alu", "achieved": kr[dom]["tflops"], "peak": leg["peak_tflops"],
                 "unit": "TFLOP/s", "frac": kr[dom]["frac"],
                 "traffic": ncu_traffic(dom, cfg, cnt.n_subgrids, kr[dom]["launches_per_step"]),
                 "peak_basis": f"{N_SM} SM x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {peaks['sm_max_mhz']:.0f} MHz "
                               f"(sm_max_mhz {peaks['source']}); work = 18 FP32-pipe ops per (vis,pixel) pair",
                 "frac_at_observed_clock": kr[dom]["frac_at_observed_clock"],
                 "hbm_frac_of_measured": kr[dom]["hbm_frac"], "hbm_peak_gbs": peaks["hbm_gbs"]}
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
-            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": workload_config(cfg), "grid_vis_per_s": n_vis / (grid_ms / 1e3),
-            "degrid_vis_per_s": n_vis / (degrid_ms / 1e3), "grid_ms": grid_ms, "degrid_ms": degrid_ms,
+    metric = METRIC if not prediction_only else "degridded (predicted) visibilities/s (4 pols each)"
+    line = {"metric": metric, "value": value, "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": warmup, "ms_per_step": ms_per_step,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "operands": OPERANDS,
+            "data": "synthetic", "config": workload_config(cfg), "grid_vis_per_s": leg.get("grid_vis_per_s"),
+            "degrid_vis_per_s": leg["degrid_vis_per_s"], "grid_ms": leg.get("grid_ms"), "degrid_ms": leg["degrid_ms"],
             "n_subgrids": int(cnt.n_subgrids), "n_vis": int(n_vis), "roofline": roofline, "kernels": kr,
-            "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks}
+            "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": leg["launches"], "clocks": clocks,
+            "other_configs": others}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -481,6 +557,8 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="wall-time target of the cpu_baseline leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true",
+                    help="skip the brief runs of configs 3, 4 and 5 that follow the config-2 headline")
     ap.add_argument("--e2e-batch", type=int, default=8192,
                     help="subgrids per batch of the plan the end-to-end leg uses (0 = same plan as the device leg)")
     ap.add_argument("--max-batch", type=int, default=0,

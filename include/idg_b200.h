@@ -11,7 +11,7 @@
  *                -> degridder (Eq. 13 :171-174)
  *
  * Conventions:
- *   Ng grid size (even), cell [rad], S = Ng*cell; L subgrid size in {32,64,96,128}; P total
+ *   Ng grid size (even), cell [rad], S = Ng*cell; L subgrid size in {32,48,64,96,128,160}; P total
  *   kernel padding in pixels; kappa_c = nu_c / 299792458.0; row r = b*n_times + t
  *   (baseline-major); u = u_m(r)*kappa_c [wavelengths].
  *   subgrid s = (b, t0, nt, c0, nc, x0, y0, wl): rows b*n_times + t0 .. +nt, channels c0 .. +nc,
@@ -50,7 +50,7 @@ extern "C" {
 
 #define IDG_OK            0
 #define IDG_EINVAL       -1   /* bad argument (null pointer, non-ascending channels, bad sizes)  */
-#define IDG_EUNSUPPORTED -2   /* subgrid size not in {32,64,96,128}                              */
+#define IDG_EUNSUPPORTED -2   /* subgrid size not in {32,48,64,96,128,160}                       */
 #define IDG_ENOMEM       -3   /* workspace too small / host allocation failed                   */
 #define IDG_ECUDA        -4   /* CUDA runtime error (message in idg_last_error)                 */
 
@@ -65,7 +65,7 @@ typedef struct idg_plan idg_plan;          /* opaque; host-owned; immutable afte
 
 typedef struct {
   int32_t grid_size;      /* Ng, even                                                            */
-  int32_t subgrid_size;   /* L in {32, 64, 96, 128}                                              */
+  int32_t subgrid_size;   /* L in {32, 48, 64, 96, 128, 160}                                     */
   int32_t padding;        /* P, total kernel padding in pixels, 0 <= P < L-1  (R8)               */
   int32_t n_stations;
   int32_t n_baselines;
@@ -77,6 +77,14 @@ typedef struct {
   double  comfort;        /* fraction of the usable span a channel range may fill (R7); 0.75     */
   int64_t max_batch_subgrids; /* subgrids processed per batch (§3.4 :259-267, R18);
                                  0 => library default                                            */
+  int32_t gridder_variant;   /* IDG_VARIANT_* of the gridder direct sum (0 = AUTO), see below    */
+  int32_t degridder_variant; /* IDG_VARIANT_* of the degridder direct sum (0 = AUTO)             */
+  int32_t positive_w;     /* != 0: rows with w < 0 are used as (-u,-v,-w) of the swapped baseline
+                             with V^dagger, so that only layers wl >= 0 exist (PAPER.md:178
+                             footnote 4, R21).  A subgrid never mixes the two kinds of row.      */
+  int32_t power_norm;     /* != 0: the imaging sandwich is divided per pixel by the Frobenius
+                             norm || M_p M_q^H ||_F (§3.3, R22); the caller corrects
+                             the image by idg_power_norm_average.  Prediction is not normalised. */
 } idg_params;
 
 /* ---- planner: visibility table -> subgrids (§2.2 :62-72, §2.4 :141-143, §3.1
@@ -206,17 +214,57 @@ IDG_API int  idg_grid_to_image(const idg_plan* plan, const void* grid_dev, const
 IDG_API int  idg_image_to_grid(const idg_plan* plan, const void* image_dev, const float* corr_dev, void* grid_dev,
                        void* cuda_stream);
 
-/* Kernel variant of the two direct-sum kernels (process-wide; kind = IDG_K_GRIDDER or
- * IDG_K_DEGRIDDER).  IDG_VARIANT_SIMT: all arithmetic on the FP32/SFU pipes (packed FFMA2).
- * IDG_VARIANT_TENSOR: the phasor matrix is generated on the SIMT pipes and the 2x2 complex MACs run
- * on the tensor cores (tcgen05, split-tf32 operands, fp32 accumulation).  Both meet the 1e-5 bar.
- * IDG_VARIANT_AUTO (the default): per launch, the tensor-core kernel when at least 80 % of its
- * 8-channel chunks carry visibilities (and the shape fits its shared-memory tables), else SIMT. */
-#define IDG_VARIANT_SIMT   0
-#define IDG_VARIANT_TENSOR 1
-#define IDG_VARIANT_AUTO   2
-IDG_API int  idg_set_kernel_variant(int kind, int variant);
-IDG_API int  idg_get_kernel_variant(int kind);
+/* Kernel variant of the two direct-sum kernels: a PLAN parameter (idg_params.gridder_variant /
+ * .degridder_variant), so two plans in one process may differ.
+ * IDG_VARIANT_AUTO (0, the default): PER SUBGRID (PAPER.md:247 footnote 7, "swap the kernel design by a
+ *   subgrid-occupancy heuristic"; :239-241), the tensor-core kernel where its operand slots are well filled
+ *   (gridder: at least 80 % of the 8-channel chunks of a table row carry visibilities; degridder: at least
+ *   48 visibilities) and the shape fits its shared-memory tables, else the SIMT kernel.  A batch is then
+ *   two launches over complementary index lists; the adder's order is untouched.
+ * IDG_VARIANT_SIMT: all arithmetic on the FP32 / SFU pipes (packed FFMA2).
+ * IDG_VARIANT_TENSOR: the phasor matrix is generated on the SIMT pipes and the 2x2 complex MACs run on the
+ *   tensor cores (tcgen05, fp32 accumulation drained into registers).  Operands are split into a head and a
+ *   remainder of 11 significant bits each: the gridder uses fp16 heads + fp16 remainders with ONE
+ *   power-of-two scale per segment of a subgrid (at most 2560 visibilities), so its absolute error is about
+ *   2^-22 of the segment's largest |component|: samples far below the segment maximum keep that ABSOLUTE
+ *   accuracy, not their relative one (tests pin this with 1e6 of dynamic range inside one subgrid).  The
+ *   degridder uses tf32 heads + tf32 remainders (relative 2^-22 per operand).
+ * IDG_VARIANT_FP64: SIMT kernels with the phase, sin/cos and accumulation in fp64 (§5.3: the
+ *   fp64 kernels are about 4.5x slower; §4.1 :289-293 accuracy experiment); inputs and the subgrid stack
+ *   stay complex64 on the idg_grid / idg_degrid path, the *_f64 stage calls below keep fp64 end to end.
+ * All but FP64 meet the 1e-5 bar with margin; FP64 is for accuracy studies. */
+#define IDG_VARIANT_AUTO   0
+#define IDG_VARIANT_SIMT   1
+#define IDG_VARIANT_TENSOR 2
+#define IDG_VARIANT_FP64   3
+
+/* Which kernels the direct-sum step `kind` (IDG_K_GRIDDER or IDG_K_DEGRIDDER) has launched in this process
+ * since the last reset, as a bit mask: bit 0 SIMT, bit 1 / 2 / 4 tensor-core with 1 / 2 / 4 compute groups
+ * per CTA (the gridder picks by shared-memory fit; the degridder always runs 2), bit 8 fp64.  reset != 0
+ * clears the mask after reading.  For the tests, which must know what they exercised. */
+#define IDG_KMASK_SIMT   (1 << 0)
+#define IDG_KMASK_TC(ng) (1 << (ng))
+#define IDG_KMASK_FP64   (1 << 8)
+IDG_API int  idg_kernel_config_mask(int kind, int reset);
+
+/* fp64 stage calls: the two direct sums with their A-term /
+ * taper step in double precision from the same complex64 / float32 inputs.
+ *   idg_grid_subgrids_f64  : subgrids_dev [count, 4, L, L] complex128, stage IDG_STAGE_GRIDDER only
+ *   idg_degrid_subgrids_f64: subgrids_dev [count, 4, L, L] complex128 in, vis_dev [n_rows, n_chan, 4]
+ *                            complex128 out (planned visibilities of the range only) */
+IDG_API int  idg_grid_subgrids_f64(const idg_plan* plan, int64_t first, int64_t count, const void* vis_dev,
+                           const void* aterms_dev, const float* taper_dev, void* subgrids_dev,
+                           void* cuda_stream);
+IDG_API int  idg_degrid_subgrids_f64(const idg_plan* plan, int64_t first, int64_t count, const void* subgrids_dev,
+                             const void* aterms_dev, const float* taper_dev, void* vis_dev,
+                             void* cuda_stream);
+
+/* Weighted average over the subgrids of the power-normalisation factor 1 / || M_p M_q^H ||_F, weights =
+ * visibilities per subgrid ("the final image must then be corrected by the weighted average
+ * of this normalisation factor across all subgrids", R22).  avg_dev [L, L] float64, overwritten.
+ * Works for any plan (power_norm on or off); synchronises the stream. */
+IDG_API int  idg_power_norm_average(const idg_plan* plan, const void* aterms_dev, double* avg_dev,
+                            void* cuda_stream);
 
 /* Empirical ALU peaks of the current device, measured the way the paper measures its Table 1
  * (§5.1 :339-351): register-only loops timed with the SM cycle counter.  Synchronous.
@@ -224,7 +272,7 @@ IDG_API int  idg_get_kernel_variant(int kind);
  * [2] MUFU.EX2 lane-ops, [3] sin+cos pairs (__sincosf), [4] (visibility, pixel) pairs of the
  * gridder's instruction mix (phase FFMA + __sincosf + 8 FFMA2 per pair), [5] the same mix with
  * 16 scalar FFMA, [6] pairs of the operand-generation mix alone (phase FFMA + __sincosf + split of
- * cos and sin into a tf32 head and an exact remainder: what is left on the SIMT pipes when the
+ * cos and sin into a tf32 head and an exact remainder, the round-1 operand format: what is left on the SIMT pipes when the
  * MACs go to the tensor cores).  These are the
  * denominators of the ALU roofline. */
 IDG_API int  idg_measure_alu_peaks(double* out_host);

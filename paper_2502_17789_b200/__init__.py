@@ -26,7 +26,8 @@ SYMBOLS = (
     "idg_grid", "idg_grid_weighted", "idg_degrid", "idg_host_arena_bytes", "idg_host_traffic_bytes", "idg_grid_host", "idg_degrid_host",
     "idg_grid_subgrids", "idg_degrid_subgrids", "idg_subgrid_fft", "idg_adder", "idg_splitter",
     "idg_closure_workspace_bytes", "idg_grid_to_image", "idg_image_to_grid",
-    "idg_profile_enable", "idg_profile_read", "idg_set_kernel_variant", "idg_get_kernel_variant",
+    "idg_grid_subgrids_f64", "idg_degrid_subgrids_f64", "idg_power_norm_average",
+    "idg_profile_enable", "idg_profile_read", "idg_kernel_config_mask",
     "idg_measure_alu_peaks", "idg_launch_count", "idg_last_error", "idg_version",
 )
 KERNEL_KINDS = ("gridder", "fft", "adder", "splitter", "ifft", "degridder")
@@ -43,6 +44,8 @@ class _Params(ctypes.Structure):
         ("n_chan", ctypes.c_int32), ("aterm_period", ctypes.c_int32),
         ("cell_size", ctypes.c_double), ("w_step", ctypes.c_double), ("comfort", ctypes.c_double),
         ("max_batch_subgrids", ctypes.c_int64),
+        ("gridder_variant", ctypes.c_int32), ("degridder_variant", ctypes.c_int32),
+        ("positive_w", ctypes.c_int32), ("power_norm", ctypes.c_int32),
     ]
 
 
@@ -104,10 +107,14 @@ def load_library() -> ctypes.CDLL:
     lib.idg_profile_enable.restype = ctypes.c_int
     lib.idg_profile_read.argtypes = [vp, vp]
     lib.idg_profile_read.restype = ctypes.c_int
-    lib.idg_set_kernel_variant.argtypes = [ctypes.c_int, ctypes.c_int]
-    lib.idg_set_kernel_variant.restype = ctypes.c_int
-    lib.idg_get_kernel_variant.argtypes = [ctypes.c_int]
-    lib.idg_get_kernel_variant.restype = ctypes.c_int
+    lib.idg_kernel_config_mask.argtypes = [ctypes.c_int, ctypes.c_int]
+    lib.idg_kernel_config_mask.restype = ctypes.c_int
+    lib.idg_grid_subgrids_f64.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
+    lib.idg_grid_subgrids_f64.restype = ctypes.c_int
+    lib.idg_degrid_subgrids_f64.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
+    lib.idg_degrid_subgrids_f64.restype = ctypes.c_int
+    lib.idg_power_norm_average.argtypes = [vp, vp, vp, vp]
+    lib.idg_power_norm_average.restype = ctypes.c_int
     lib.idg_measure_alu_peaks.argtypes = [vp]
     lib.idg_measure_alu_peaks.restype = ctypes.c_int
     lib.idg_launch_count.argtypes = []
@@ -159,11 +166,21 @@ class PlanCounts:
     n_vis_dropped: int
 
 
+VARIANT_AUTO, VARIANT_SIMT, VARIANT_TENSOR, VARIANT_FP64 = 0, 1, 2, 3
+KMASK_SIMT, KMASK_FP64 = 1 << 0, 1 << 8
+
+
+def kmask_tc(ng: int) -> int:
+    """Bit of idg_kernel_config_mask for the tensor-core kernel with `ng` compute groups per CTA."""
+    return 1 << ng
+
+
 class Plan:
     """Owner of an `idg_plan*` (idg_plan_create / idg_plan_destroy)."""
 
     def __init__(self, *, grid_size, subgrid_size, padding, cell_size, w_step, n_stations, n_times, n_chan,
-                 aterm_period, uvw_m, freqs, baselines, comfort=0.75, max_batch_subgrids=0):
+                 aterm_period, uvw_m, freqs, baselines, comfort=0.75, max_batch_subgrids=0,
+                 gridder_variant=VARIANT_AUTO, degridder_variant=VARIANT_AUTO, positive_w=False, power_norm=False):
         lib = load_library()
         uvw_m = np.ascontiguousarray(uvw_m, dtype=np.float64)
         freqs = np.ascontiguousarray(freqs, dtype=np.float64)
@@ -172,13 +189,19 @@ class Plan:
         if uvw_m.shape != (n_bl * n_times, 3) or freqs.shape != (n_chan,) or baselines.shape != (n_bl, 2):
             raise ValueError("uvw_m must be [n_bl*n_times,3], freqs [n_chan], baselines [n_bl,2]")
         self.params = _Params(grid_size, subgrid_size, padding, n_stations, n_bl, n_times, n_chan, aterm_period,
-                              cell_size, w_step, comfort, max_batch_subgrids)
+                              cell_size, w_step, comfort, max_batch_subgrids, int(gridder_variant),
+                              int(degridder_variant), int(bool(positive_w)), int(bool(power_norm)))
         handle = ctypes.c_void_p()
         _check(lib.idg_plan_create(ctypes.byref(self.params), uvw_m.ctypes.data, freqs.ctypes.data,
                                    baselines.ctypes.data, ctypes.byref(handle)), "idg_plan_create")
         self._h = handle
         self.n_rows = n_bl * n_times
+        self.n_chan = n_chan
+        self.n_stations = n_stations
+        self.subgrid_size = subgrid_size
+        self.grid_size = grid_size
         self.n_intervals = -(-n_times // aterm_period)
+        self._counts = None
 
     def __del__(self):
         h = getattr(self, "_h", None)
@@ -191,10 +214,13 @@ class Plan:
         return self._h
 
     def counts(self) -> PlanCounts:
-        n, w, wl, pl, dr = ctypes.c_int64(), ctypes.c_int32(), ctypes.c_int32(), ctypes.c_int64(), ctypes.c_int64()
-        _check(load_library().idg_plan_counts(self._h, ctypes.byref(n), ctypes.byref(w), ctypes.byref(wl),
-                                              ctypes.byref(pl), ctypes.byref(dr)), "idg_plan_counts")
-        return PlanCounts(n.value, w.value, wl.value, pl.value, dr.value)
+        if self._counts is None:
+            n, w, wl, pl, dr = (ctypes.c_int64(), ctypes.c_int32(), ctypes.c_int32(), ctypes.c_int64(),
+                                ctypes.c_int64())
+            _check(load_library().idg_plan_counts(self._h, ctypes.byref(n), ctypes.byref(w), ctypes.byref(wl),
+                                                  ctypes.byref(pl), ctypes.byref(dr)), "idg_plan_counts")
+            self._counts = PlanCounts(n.value, w.value, wl.value, pl.value, dr.value)
+        return self._counts
 
     def export(self) -> np.ndarray:
         n = self.counts().n_subgrids
@@ -218,44 +244,94 @@ class Plan:
     def closure_workspace_bytes(self) -> int:
         return int(load_library().idg_closure_workspace_bytes(self._h))
 
+    # ---- sizes of the arrays the C ABI takes (it sees only pointers: the binding checks dtype and size)
+    def vis_numel(self) -> int:
+        return self.n_rows * self.n_chan * 4
 
-def plan_from_config(cfg, uvw_m, freqs, baselines, max_batch_subgrids=0) -> Plan:
-    """Convenience: a Plan from a `synth.Config`-like object (attribute names as in include/idg_b200.h)."""
+    def aterms_numel(self) -> int:
+        L = self.subgrid_size
+        return self.n_stations * self.n_intervals * L * L * 4
+
+    def grid_numel(self) -> int:
+        return self.counts().n_wlayers * 4 * self.grid_size * self.grid_size
+
+
+def plan_from_config(cfg, uvw_m, freqs, baselines, max_batch_subgrids=0, **kw) -> Plan:
+    """Convenience: a Plan from a `synth.Config`-like object (attribute names as in include/idg_b200.h);
+    kw: gridder_variant, degridder_variant, positive_w, power_norm."""
     return Plan(grid_size=cfg.grid_size, subgrid_size=cfg.subgrid_size, padding=cfg.padding,
                 cell_size=cfg.cell_size, w_step=cfg.w_step, n_stations=cfg.n_stations, n_times=cfg.n_times,
                 n_chan=cfg.n_chan, aterm_period=cfg.aterm_period, uvw_m=uvw_m, freqs=freqs, baselines=baselines,
-                comfort=cfg.comfort, max_batch_subgrids=max_batch_subgrids)
+                comfort=cfg.comfort, max_batch_subgrids=max_batch_subgrids, **kw)
+
+
+_DTYPES = {"c64": ("complex64",), "c128": ("complex128",), "f32": ("float32",), "f64": ("float64",)}
+
+
+def _expect(t, kind: str, numel: int, what: str, at_least: bool = False) -> None:
+    """dtype and element count of an array handed to the C ABI (which cannot see either); `at_least` for
+    buffers of which a call may use only the leading part."""
+    name = str(t.dtype).replace("torch.", "")
+    if name not in _DTYPES[kind]:
+        raise ValueError(f"{what}: dtype {name}, expected {_DTYPES[kind][0]}")
+    n = int(t.numel()) if hasattr(t, "numel") else int(t.size)
+    if n != numel and not (at_least and n > numel):
+        raise ValueError(f"{what}: {n} elements, expected {numel}")
+
+
+def _expect_common(plan: Plan, vis=None, aterms=None, taper=None, grid=None, vis_kind="c64") -> None:
+    L = plan.subgrid_size
+    if vis is not None:
+        _expect(vis, vis_kind, plan.vis_numel(), "vis [n_rows, n_chan, 4]")
+    if aterms is not None:
+        _expect(aterms, "c64", plan.aterms_numel(), "aterms [n_stations, n_intervals, L, L, 2, 2]")
+    if taper is not None:
+        _expect(taper, "f32", L * L, "taper [L, L]")
+    if grid is not None:
+        _expect(grid, "c64", plan.grid_numel(), "grid [n_wlayers, 4, Ng, Ng]")
+
+
+def _nbytes(t) -> int:
+    return t.numel() * t.element_size()
 
 
 def grid(plan: Plan, vis, aterms, taper, grid_out, workspace, stream=None) -> None:
     """idg_grid: accumulate all subgrids of the plan into grid_out [W,4,Ng,Ng] complex64."""
     _need_cuda(vis, aterms, taper, grid_out, workspace)
+    _expect_common(plan, vis, aterms, taper, grid_out)
     _check(load_library().idg_grid(plan.handle, _ptr(vis), _ptr(aterms), _ptr(taper), _ptr(grid_out),
-                                   _ptr(workspace), workspace.numel() * workspace.element_size(),
-                                   _stream_ptr(stream)), "idg_grid")
+                                   _ptr(workspace), _nbytes(workspace), _stream_ptr(stream)), "idg_grid")
 
 
 def grid_weighted(plan: Plan, vis, weights, aterms, taper, grid_out, workspace, stream=None) -> None:
     """idg_grid_weighted: as grid(), with vis[r, c, :] * weights[r, c] (float32) applied at load."""
     _need_cuda(vis, weights, aterms, taper, grid_out, workspace)
+    _expect_common(plan, vis, aterms, taper, grid_out)
+    _expect(weights, "f32", plan.n_rows * plan.n_chan, "weights [n_rows, n_chan]")
     _check(load_library().idg_grid_weighted(plan.handle, _ptr(vis), _ptr(weights), _ptr(aterms), _ptr(taper),
-                                            _ptr(grid_out), _ptr(workspace),
-                                            workspace.numel() * workspace.element_size(), _stream_ptr(stream)),
-           "idg_grid_weighted")
+                                            _ptr(grid_out), _ptr(workspace), _nbytes(workspace),
+                                            _stream_ptr(stream)), "idg_grid_weighted")
 
 
 def grid_to_image(plan: Plan, grid_in, image_out, workspace, corr=None, stream=None) -> None:
     """idg_grid_to_image (w-stacking closure, outside the hot path): image_out [4,Ng,Ng] complex64."""
     _need_cuda(grid_in, image_out, workspace, *(() if corr is None else (corr,)))
+    _expect_common(plan, grid=grid_in)
+    _expect(image_out, "c64", 4 * plan.grid_size ** 2, "image [4, Ng, Ng]")
+    if corr is not None:
+        _expect(corr, "f32", plan.grid_size ** 2, "corr [Ng, Ng]")
     _check(load_library().idg_grid_to_image(plan.handle, _ptr(grid_in), None if corr is None else _ptr(corr),
-                                            _ptr(image_out), _ptr(workspace),
-                                            workspace.numel() * workspace.element_size(), _stream_ptr(stream)),
-           "idg_grid_to_image")
+                                            _ptr(image_out), _ptr(workspace), _nbytes(workspace),
+                                            _stream_ptr(stream)), "idg_grid_to_image")
 
 
 def image_to_grid(plan: Plan, image_in, grid_out, corr=None, stream=None) -> None:
     """idg_image_to_grid: grid_out [W,4,Ng,Ng] complex64 is overwritten."""
     _need_cuda(image_in, grid_out, *(() if corr is None else (corr,)))
+    _expect_common(plan, grid=grid_out)
+    _expect(image_in, "c64", 4 * plan.grid_size ** 2, "image [4, Ng, Ng]")
+    if corr is not None:
+        _expect(corr, "f32", plan.grid_size ** 2, "corr [Ng, Ng]")
     _check(load_library().idg_image_to_grid(plan.handle, _ptr(image_in), None if corr is None else _ptr(corr),
                                             _ptr(grid_out), _stream_ptr(stream)), "idg_image_to_grid")
 
@@ -263,56 +339,93 @@ def image_to_grid(plan: Plan, image_in, grid_out, corr=None, stream=None) -> Non
 def degrid(plan: Plan, grid_in, aterms, taper, vis_out, workspace, stream=None) -> None:
     """idg_degrid: predict every planned visibility into vis_out [n_rows,n_chan,4] complex64."""
     _need_cuda(vis_out, aterms, taper, grid_in, workspace)
+    _expect_common(plan, vis_out, aterms, taper, grid_in)
     _check(load_library().idg_degrid(plan.handle, _ptr(grid_in), _ptr(aterms), _ptr(taper), _ptr(vis_out),
-                                     _ptr(workspace), workspace.numel() * workspace.element_size(),
-                                     _stream_ptr(stream)), "idg_degrid")
+                                     _ptr(workspace), _nbytes(workspace), _stream_ptr(stream)), "idg_degrid")
 
 
 def grid_host(plan: Plan, vis, aterms, taper, grid_io, arena, stream=None) -> None:
     """idg_grid_host: host buffers in, host grid accumulated; copies run inside the call."""
     _need_cuda(arena)
+    _expect_common(plan, vis, aterms, taper, grid_io)
     _check(load_library().idg_grid_host(plan.handle, _ptr(vis), _ptr(aterms), _ptr(taper), _ptr(grid_io),
-                                        _ptr(arena), arena.numel() * arena.element_size(),
-                                        _stream_ptr(stream)), "idg_grid_host")
+                                        _ptr(arena), _nbytes(arena), _stream_ptr(stream)), "idg_grid_host")
 
 
 def degrid_host(plan: Plan, grid_in, aterms, taper, vis_io, arena, stream=None) -> None:
     """idg_degrid_host: host buffers in, host visibilities out."""
     _need_cuda(arena)
+    _expect_common(plan, vis_io, aterms, taper, grid_in)
     _check(load_library().idg_degrid_host(plan.handle, _ptr(grid_in), _ptr(aterms), _ptr(taper), _ptr(vis_io),
-                                          _ptr(arena), arena.numel() * arena.element_size(),
-                                          _stream_ptr(stream)), "idg_degrid_host")
+                                          _ptr(arena), _nbytes(arena), _stream_ptr(stream)), "idg_degrid_host")
 
 
 def grid_subgrids(plan: Plan, first, count, vis, aterms, taper, subgrids_out, stage=STAGE_FFT, stream=None) -> None:
     _need_cuda(vis, aterms, taper, subgrids_out)
+    _expect_common(plan, vis, aterms, taper)
+    _expect(subgrids_out, "c64", count * 4 * plan.subgrid_size ** 2, "subgrids [count, 4, L, L]", at_least=True)
     _check(load_library().idg_grid_subgrids(plan.handle, first, count, _ptr(vis), _ptr(aterms), _ptr(taper),
                                             _ptr(subgrids_out), stage, _stream_ptr(stream)), "idg_grid_subgrids")
 
 
 def degrid_subgrids(plan: Plan, first, count, subgrids_in, aterms, taper, vis_out, stream=None) -> None:
     _need_cuda(vis_out, aterms, taper, subgrids_in)
+    _expect_common(plan, vis_out, aterms, taper)
+    _expect(subgrids_in, "c64", count * 4 * plan.subgrid_size ** 2, "subgrids [count, 4, L, L]", at_least=True)
     _check(load_library().idg_degrid_subgrids(plan.handle, first, count, _ptr(subgrids_in), _ptr(aterms),
                                               _ptr(taper), _ptr(vis_out), _stream_ptr(stream)),
            "idg_degrid_subgrids")
+
+
+def grid_subgrids_f64(plan: Plan, first, count, vis, aterms, taper, subgrids_out, stream=None) -> None:
+    """idg_grid_subgrids_f64: the fp64 gridder + A-term / taper; subgrids_out [count,4,L,L] complex128."""
+    _need_cuda(vis, aterms, taper, subgrids_out)
+    _expect_common(plan, vis, aterms, taper)
+    _expect(subgrids_out, "c128", count * 4 * plan.subgrid_size ** 2, "subgrids [count, 4, L, L]", at_least=True)
+    _check(load_library().idg_grid_subgrids_f64(plan.handle, first, count, _ptr(vis), _ptr(aterms), _ptr(taper),
+                                                _ptr(subgrids_out), _stream_ptr(stream)), "idg_grid_subgrids_f64")
+
+
+def degrid_subgrids_f64(plan: Plan, first, count, subgrids_in, aterms, taper, vis_out, stream=None) -> None:
+    """idg_degrid_subgrids_f64: complex128 subgrids in, complex128 visibilities out."""
+    _need_cuda(vis_out, aterms, taper, subgrids_in)
+    _expect_common(plan, vis_out, aterms, taper, vis_kind="c128")
+    _expect(subgrids_in, "c128", count * 4 * plan.subgrid_size ** 2, "subgrids [count, 4, L, L]", at_least=True)
+    _check(load_library().idg_degrid_subgrids_f64(plan.handle, first, count, _ptr(subgrids_in), _ptr(aterms),
+                                                  _ptr(taper), _ptr(vis_out), _stream_ptr(stream)),
+           "idg_degrid_subgrids_f64")
+
+
+def power_norm_average(plan: Plan, aterms, avg_out, stream=None) -> None:
+    """idg_power_norm_average: avg_out [L, L] float64, the visibility-weighted mean of 1 / ||M_p M_q^H||_F."""
+    _need_cuda(aterms, avg_out)
+    _expect_common(plan, aterms=aterms)
+    _expect(avg_out, "f64", plan.subgrid_size ** 2, "avg [L, L]")
+    _check(load_library().idg_power_norm_average(plan.handle, _ptr(aterms), _ptr(avg_out), _stream_ptr(stream)),
+           "idg_power_norm_average")
 
 
 def subgrid_fft(subgrid_size, planes, direction, stream=None) -> None:
     """idg_subgrid_fft: planes [..., L, L] complex64, transformed in place."""
     _need_cuda(planes)
     n_planes = planes.numel() // (subgrid_size * subgrid_size)
+    _expect(planes, "c64", n_planes * subgrid_size * subgrid_size, "planes [..., L, L]")
     _check(load_library().idg_subgrid_fft(subgrid_size, n_planes, _ptr(planes), direction, _stream_ptr(stream)),
            "idg_subgrid_fft")
 
 
 def adder(plan: Plan, first, count, subgrids, grid_io, stream=None) -> None:
     _need_cuda(subgrids, grid_io)
+    _expect_common(plan, grid=grid_io)
+    _expect(subgrids, "c64", count * 4 * plan.subgrid_size ** 2, "subgrids [count, 4, L, L]", at_least=True)
     _check(load_library().idg_adder(plan.handle, first, count, _ptr(subgrids), _ptr(grid_io), _stream_ptr(stream)),
            "idg_adder")
 
 
 def splitter(plan: Plan, first, count, grid_in, subgrids_out, stream=None) -> None:
     _need_cuda(subgrids_out, grid_in)
+    _expect_common(plan, grid=grid_in)
+    _expect(subgrids_out, "c64", count * 4 * plan.subgrid_size ** 2, "subgrids [count, 4, L, L]", at_least=True)
     _check(load_library().idg_splitter(plan.handle, first, count, _ptr(grid_in), _ptr(subgrids_out),
                                        _stream_ptr(stream)), "idg_splitter")
 
@@ -329,16 +442,12 @@ def profile_read() -> dict:
     return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(KERNEL_KINDS)}
 
 
-VARIANT_SIMT, VARIANT_TENSOR, VARIANT_AUTO = 0, 1, 2
-
-
-def set_kernel_variant(kind: str, variant: int) -> None:
-    """idg_set_kernel_variant: kind in ("gridder", "degridder"); variant VARIANT_SIMT | VARIANT_TENSOR | VARIANT_AUTO."""
-    _check(load_library().idg_set_kernel_variant(KERNEL_KINDS.index(kind), int(variant)), "idg_set_kernel_variant")
-
-
-def get_kernel_variant(kind: str) -> int:
-    return int(load_library().idg_get_kernel_variant(KERNEL_KINDS.index(kind)))
+def kernel_config_mask(kind: str, reset: bool = False) -> int:
+    """idg_kernel_config_mask: which kernels the direct-sum step `kind` ("gridder" | "degridder") launched."""
+    m = int(load_library().idg_kernel_config_mask(KERNEL_KINDS.index(kind), 1 if reset else 0))
+    if m < 0:
+        _check(m, "idg_kernel_config_mask")
+    return m
 
 
 def measure_alu_peaks() -> dict:

@@ -203,13 +203,10 @@ cudaError_t launch_adder(const int32_t* meta, const DeviceCsr& csr, int64_t firs
   if (csr.n_slots > 0 && (!csr.partials || !csr.counters)) return cudaErrorInvalidValue;
   dim3 grid_dim(static_cast<unsigned>(csr.n_segs), 1, 1);
   constexpr size_t smem = static_cast<size_t>(kAdderStages) * 4 * (kTile * kTile / kAdderThreads) * kAdderThreads * sizeof(float2);
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(adder_kernel<kAdderThreads>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         static_cast<int>(smem));
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  // per launch: the attribute belongs to the (function, device) pair and the call is cheap
+  cudaError_t e = cudaFuncSetAttribute(adder_kernel<kAdderThreads>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       static_cast<int>(smem));
+  if (e != cudaSuccess) return e;
   adder_kernel<kAdderThreads><<<grid_dim, kAdderThreads, smem, stream>>>(meta, csr.tile_ids, csr.segs, csr.items, first, L,
                                                                       Ng, tiles_x, tiles_y, subgrids, grid,
                                                                       csr.partials, csr.counters);

@@ -15,10 +15,11 @@ namespace idg {
 
 static thread_local std::string g_last_error;
 static std::atomic<int64_t> g_launches{0};
-static std::atomic<int> g_variant[IDG_K_COUNT] = {IDG_VARIANT_AUTO, 0, 0, 0, 0, IDG_VARIANT_AUTO};
+static std::atomic<int> g_kmask[IDG_K_COUNT];        // which direct-sum kernels ran (idg_kernel_config_mask)
 
 void set_error(const std::string& msg) { g_last_error = msg; }
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+void note_kernel(int kind, int bit) { g_kmask[kind].fetch_or(bit, std::memory_order_relaxed); }
 
 namespace {
 
@@ -97,10 +98,28 @@ void free_csr(DeviceCsr* c) {
   *c = DeviceCsr{};
 }
 
+cudaError_t upload_split(const KernelSplit& sp, DeviceSplit* out) {
+  *out = DeviceSplit{};
+  out->variant = sp.variant;
+  out->n_tensor = static_cast<int32_t>(sp.tensor.size());
+  out->n_simt = static_cast<int32_t>(sp.simt.size());
+  if (sp.tensor.empty() || sp.simt.empty()) return cudaSuccess;      // one launch over the whole range: no lists
+  cudaError_t e = upload(sp.tensor, &out->tensor);
+  if (e != cudaSuccess) return e;
+  return upload(sp.simt, &out->simt);
+}
+
+void free_split(DeviceSplit* s) {
+  cudaFree(s->tensor); cudaFree(s->simt);
+  *s = DeviceSplit{};
+}
+
 void free_device_state(DeviceState* d) {
   if (!d) return;
   cudaFree(d->uvw); cudaFree(d->kappa); cudaFree(d->meta); cudaFree(d->nprime);
   for (auto& c : d->batch_csr) free_csr(&c);
+  for (auto& c : d->batch_grid_split) free_split(&c);
+  for (auto& c : d->batch_degrid_split) free_split(&c);
   cudaFree(d->adder_partials); cudaFree(d->adder_counters);
   closure_plan_destroy(d->closure_fft);
   delete d;
@@ -109,9 +128,17 @@ void free_device_state(DeviceState* d) {
 // Uploads the plan metadata on first use (the only device memory the library owns).
 int ensure_device(const idg_plan* plan, const DeviceState** out) {
   std::lock_guard<std::mutex> lock(plan->mu);
-  if (plan->dev) { *out = plan->dev; return IDG_OK; }
   int dev = 0;
   IDG_CUDA(cudaGetDevice(&dev));
+  if (plan->dev) {
+    if (plan->dev->device != dev) {
+      set_error("the plan's metadata lives on device " + std::to_string(plan->dev->device) + " but the current device is " +
+                std::to_string(dev) + " (one plan per device)");
+      return IDG_EINVAL;
+    }
+    *out = plan->dev;
+    return IDG_OK;
+  }
   cudaDeviceProp prop;
   IDG_CUDA(cudaGetDeviceProperties(&prop, dev));
   if (prop.major != 10) {
@@ -140,10 +167,14 @@ int ensure_device(const idg_plan* plan, const DeviceState** out) {
     return cuda_fail(e, "plan upload");
   }
   d->batch_csr.resize(plan->batches.size());
+  d->batch_grid_split.resize(plan->batches.size());
+  d->batch_degrid_split.resize(plan->batches.size());
   for (size_t i = 0; i < plan->batches.size(); ++i) {
-    if ((e = upload_csr(plan->batches[i].csr, &d->batch_csr[i])) != cudaSuccess) {
+    if ((e = upload_csr(plan->batches[i].csr, &d->batch_csr[i])) != cudaSuccess ||
+        (e = upload_split(plan->batches[i].grid_split, &d->batch_grid_split[i])) != cudaSuccess ||
+        (e = upload_split(plan->batches[i].degrid_split, &d->batch_degrid_split[i])) != cudaSuccess) {
       free_device_state(d);
-      return cuda_fail(e, "plan upload (tile lists)");
+      return cuda_fail(e, "plan upload (tile and kernel lists)");
     }
   }
   // the adder's scratch is shared by the batches (they run one after another on one stream)
@@ -166,6 +197,9 @@ SubgridJob make_job(const idg_plan* plan, const DeviceState* d, int64_t first, i
   j.aterms = static_cast<const float4*>(aterms);
   j.taper = taper;
   j.weights = nullptr;
+  j.index = nullptr;
+  j.power_norm = plan->par.power_norm;
+  j.dkappa = plan->dkappa;
   j.first = first; j.count = count;
   j.subgrid_size = plan->par.subgrid_size; j.grid_size = plan->par.grid_size;
   j.n_times = plan->par.n_times; j.n_chan = plan->par.n_chan; j.n_intervals = plan->n_intervals;
@@ -174,47 +208,57 @@ SubgridJob make_job(const idg_plan* plan, const DeviceState* d, int64_t first, i
   return j;
 }
 
-// Fraction of the tensor-core gridder's 8-channel chunks that carry visibilities, over a subgrid range:
-// rows of few channels leave most of a chunk empty, and the SIMT kernel, which has no padding, wins.
-double tensor_fill(const idg_plan* plan, int64_t first, int64_t count) {
-  double used = 0.0, padded = 0.0;
-  for (int64_t s = first; s < first + count; ++s) {
-    const int32_t* m = &plan->sub[s * 8];
-    used += static_cast<double>(m[2]) * m[4];
-    padded += static_cast<double>(m[2]) * ((m[4] + 7) / 8 * 8);
+// The direct-sum step of one range of subgrids with the plan's kernel variant.  Under IDG_VARIANT_AUTO the
+// choice is per SUBGRID (PAPER.md:247 fn 7): `sp` says how many subgrids take which kernel and, when both
+// kinds occur, holds the two complementary index lists on the device.
+cudaError_t run_gridder(SubgridJob job, const DeviceSplit& sp, const float4* vis, float2* out, cudaStream_t stream) {
+  switch (sp.variant) {
+    case IDG_VARIANT_SIMT:   return launch_gridder(job, vis, out, stream);
+    case IDG_VARIANT_TENSOR: return launch_gridder_tc(job, vis, out, stream);
+    case IDG_VARIANT_FP64:   return launch_gridder_f64(job, vis, out, nullptr, stream);
+    default: break;
   }
-  return padded > 0.0 ? used / padded : 0.0;
+  if (sp.n_simt == 0) return launch_gridder_tc(job, vis, out, stream);
+  if (sp.n_tensor == 0) return launch_gridder(job, vis, out, stream);
+  job.index = sp.tensor; job.count = sp.n_tensor;
+  cudaError_t e = launch_gridder_tc(job, vis, out, stream);
+  if (e != cudaSuccess) return e;
+  job.index = sp.simt; job.count = sp.n_simt;
+  return launch_gridder(job, vis, out, stream);
 }
 
-// The same for the tensor-core degridder, whose MMA rows are tiles of 128 visibilities.
-double tensor_fill_degrid(const idg_plan* plan, int64_t first, int64_t count) {
-  double used = 0.0, padded = 0.0;
-  for (int64_t s = first; s < first + count; ++s) {
-    const int32_t* m = &plan->sub[s * 8];
-    const int64_t k = static_cast<int64_t>(m[2]) * m[4];
-    used += static_cast<double>(k);
-    padded += static_cast<double>((k + 127) / 128 * 128);
+cudaError_t run_degridder(SubgridJob job, const DeviceSplit& sp, const float2* in, float4* vis, cudaStream_t stream) {
+  switch (sp.variant) {
+    case IDG_VARIANT_SIMT:   return launch_degridder(job, in, vis, stream);
+    case IDG_VARIANT_TENSOR: return launch_degridder_tc(job, in, vis, stream);
+    case IDG_VARIANT_FP64:   return launch_degridder_f64(job, in, nullptr, vis, nullptr, stream);
+    default: break;
   }
-  return padded > 0.0 ? used / padded : 0.0;
+  if (sp.n_simt == 0) return launch_degridder_tc(job, in, vis, stream);
+  if (sp.n_tensor == 0) return launch_degridder(job, in, vis, stream);
+  job.index = sp.tensor; job.count = sp.n_tensor;
+  cudaError_t e = launch_degridder_tc(job, in, vis, stream);
+  if (e != cudaSuccess) return e;
+  job.index = sp.simt; job.count = sp.n_simt;
+  return launch_degridder(job, in, vis, stream);
 }
 
-constexpr double kTensorFillMin = 0.8;
+// The same for an arbitrary range (stage-level test hooks): the lists are built and uploaded for the call and
+// freed after a stream synchronisation.
+struct RangeSplit {
+  DeviceSplit d;
+  bool owned = false;
+  ~RangeSplit() { if (owned) free_split(&d); }
+  cudaError_t init(const idg_plan* plan, int64_t first, int64_t count, int direction) {
+    KernelSplit sp;
+    split_kernels(plan, first, count, direction, &sp);
+    owned = true;
+    return upload_split(sp, &d);
+  }
+  bool mixed() const { return d.tensor != nullptr; }
+};
 
-cudaError_t run_degridder(const idg_plan* plan, const SubgridJob& job, const float2* in, float4* vis,
-                          cudaStream_t stream) {
-  int v = g_variant[IDG_K_DEGRIDDER].load();
-  if (v == IDG_VARIANT_AUTO)
-    v = tensor_fill_degrid(plan, job.first, job.count) >= kTensorFillMin ? IDG_VARIANT_TENSOR : IDG_VARIANT_SIMT;
-  return v == IDG_VARIANT_TENSOR ? launch_degridder_tc(job, in, vis, stream) : launch_degridder(job, in, vis, stream);
-}
-
-cudaError_t run_gridder(const idg_plan* plan, const SubgridJob& job, const float4* vis, float2* out,
-                        cudaStream_t stream) {
-  int v = g_variant[IDG_K_GRIDDER].load();
-  if (v == IDG_VARIANT_AUTO)
-    v = tensor_fill(plan, job.first, job.count) >= kTensorFillMin ? IDG_VARIANT_TENSOR : IDG_VARIANT_SIMT;
-  return v == IDG_VARIANT_TENSOR ? launch_gridder_tc(job, vis, out, stream) : launch_gridder(job, vis, out, stream);
-}
+bool subgrid_size_ok(int L) { return L == 32 || L == 48 || L == 64 || L == 96 || L == 128 || L == 160; }
 
 bool range_ok(const idg_plan* plan, int64_t first, int64_t count) {
   return first >= 0 && count >= 0 && first + count <= plan->n_subgrids;
@@ -240,9 +284,15 @@ int idg_plan_create(const idg_params* params, const double* uvw_m_host, const do
   }
   *out = nullptr;
   const idg_params& p = *params;
-  if (p.subgrid_size != 32 && p.subgrid_size != 64 && p.subgrid_size != 96 && p.subgrid_size != 128) {
-    set_error("idg_plan_create: subgrid_size must be 32, 64, 96 or 128");
+  if (!subgrid_size_ok(p.subgrid_size)) {
+    set_error("idg_plan_create: subgrid_size must be 32, 48, 64, 96, 128 or 160");
     return IDG_EUNSUPPORTED;
+  }
+  for (int v : {p.gridder_variant, p.degridder_variant}) {
+    if (v != IDG_VARIANT_AUTO && v != IDG_VARIANT_SIMT && v != IDG_VARIANT_TENSOR && v != IDG_VARIANT_FP64) {
+      set_error("idg_plan_create: kernel variant must be IDG_VARIANT_AUTO, _SIMT, _TENSOR or _FP64");
+      return IDG_EINVAL;
+    }
   }
   if (p.grid_size < p.subgrid_size || (p.grid_size & 1) || p.padding < 0 || p.padding >= p.subgrid_size - 1 ||
       p.n_stations < 1 || p.n_baselines < 0 || p.n_times < 1 || p.n_chan < 1 || p.aterm_period < 1 ||
@@ -333,7 +383,7 @@ int grid_batch(const idg_plan* plan, const DeviceState* d, size_t i, const void*
   SubgridJob job = make_job(plan, d, bt.first, bt.count, aterms_dev, taper_dev);
   job.weights = weights_dev;
   { ProfScope ps(IDG_K_GRIDDER, stream);
-    IDG_CUDA(run_gridder(plan, job, static_cast<const float4*>(vis_dev), stack, stream)); }
+    IDG_CUDA(run_gridder(job, d->batch_grid_split[i], static_cast<const float4*>(vis_dev), stack, stream)); }
   { ProfScope ps(IDG_K_FFT, stream);
     IDG_CUDA(launch_subgrid_fft(L, bt.count * 4, stack, +1, stream)); }
   int rc = before_adder();
@@ -354,7 +404,7 @@ int degrid_batch(const idg_plan* plan, const DeviceState* d, size_t i, const voi
   { ProfScope ps(IDG_K_IFFT, stream);
     IDG_CUDA(launch_split_ifft(d->meta, bt.first, bt.count, L, Ng, static_cast<const float2*>(grid_dev), stack, stream)); }
   { ProfScope ps(IDG_K_DEGRIDDER, stream);
-    IDG_CUDA(run_degridder(plan, job, stack, static_cast<float4*>(vis_dev), stream)); }
+    IDG_CUDA(run_degridder(job, d->batch_degrid_split[i], stack, static_cast<float4*>(vis_dev), stream)); }
   return IDG_OK;
 }
 
@@ -363,8 +413,8 @@ int degrid_batch(const idg_plan* plan, const DeviceState* d, size_t i, const voi
 int idg_grid_weighted(const idg_plan* plan, const void* vis_dev, const float* weights_dev, const void* aterms_dev,
                       const float* taper_dev, void* grid_dev, void* workspace_dev, size_t workspace_bytes,
                       void* cuda_stream) {
+  if (plan && plan->n_subgrids == 0) return IDG_OK;      // nothing planned (the arrays may be empty, i.e. null)
   if (!plan || !vis_dev || !aterms_dev || !taper_dev || !grid_dev) { set_error("idg_grid: null argument"); return IDG_EINVAL; }
-  if (plan->n_subgrids == 0) return IDG_OK;
   if (!workspace_dev || workspace_bytes < idg_workspace_bytes(plan, IDG_GRID)) {
     set_error("idg_grid: workspace too small (see idg_workspace_bytes)");
     return IDG_ENOMEM;
@@ -389,8 +439,8 @@ int idg_grid(const idg_plan* plan, const void* vis_dev, const void* aterms_dev, 
 
 int idg_degrid(const idg_plan* plan, const void* grid_dev, const void* aterms_dev, const float* taper_dev,
                void* vis_dev, void* workspace_dev, size_t workspace_bytes, void* cuda_stream) {
+  if (plan && plan->n_subgrids == 0) return IDG_OK;      // nothing planned (the arrays may be empty, i.e. null)
   if (!plan || !vis_dev || !aterms_dev || !taper_dev || !grid_dev) { set_error("idg_degrid: null argument"); return IDG_EINVAL; }
-  if (plan->n_subgrids == 0) return IDG_OK;
   if (!workspace_dev || workspace_bytes < idg_workspace_bytes(plan, IDG_DEGRID)) {
     set_error("idg_degrid: workspace too small (see idg_workspace_bytes)");
     return IDG_ENOMEM;
@@ -439,7 +489,9 @@ namespace {
 // download it right after the last batch that writes it, while the other batches compute.
 void ensure_row_runs(const idg_plan* plan) {
   std::lock_guard<std::mutex> lock(plan->mu);
-  if (!plan->rows_first.empty() || plan->batches.empty()) return;
+  if (!plan->rows_first.empty() || !plan->grid_rows.empty()) return;
+  plan->grid_rows.assign(plan->n_wlayers, {0, 0});         // a plan without subgrids touches no row
+  if (plan->batches.empty()) return;
   const size_t nb = plan->batches.size();
   std::vector<int32_t> first(plan->n_rows, -1), last(plan->n_rows, -1);
   for (size_t i = 0; i < nb; ++i) {
@@ -474,6 +526,21 @@ void ensure_row_runs(const idg_plan* plan) {
   }
   for (auto& gr : plan->grid_rows)
     if (gr.second <= gr.first) gr = {0, 0};
+}
+
+// Calls fn(byte offset, byte count) for the touched rows of every (layer, polarisation) plane of the master grid.
+cudaError_t for_grid_rows(const idg_plan* plan, const std::function<cudaError_t(size_t, size_t)>& fn) {
+  const size_t Ng = plan->par.grid_size;
+  for (int32_t k = 0; k < plan->n_wlayers; ++k) {
+    const auto gr = plan->grid_rows[k];
+    const size_t n = static_cast<size_t>(gr.second - gr.first) * Ng * sizeof(float2);
+    if (n == 0) continue;
+    for (int p = 0; p < 4; ++p) {
+      cudaError_t e = fn(((static_cast<size_t>(k) * 4 + p) * Ng + gr.first) * Ng * sizeof(float2), n);
+      if (e != cudaSuccess) return e;
+    }
+  }
+  return cudaSuccess;
 }
 
 // Copies the touched rows of every (layer, polarisation) plane of the master grid between host and device
@@ -527,6 +594,11 @@ struct CopyLane {
 
 int idg_host_traffic_bytes(const idg_plan* plan, int direction, int64_t* h2d_bytes, int64_t* d2h_bytes) {
   if (!plan || (direction != IDG_GRID && direction != IDG_DEGRID)) { set_error("idg_host_traffic_bytes: bad argument"); return IDG_EINVAL; }
+  if (plan->n_subgrids == 0) {                            // nothing is planned: the host calls move nothing
+    if (h2d_bytes) *h2d_bytes = 0;
+    if (d2h_bytes) *d2h_bytes = 0;
+    return IDG_OK;
+  }
   ensure_row_runs(plan);
   const idg_params& p = plan->par;
   const int64_t L = p.subgrid_size;
@@ -553,6 +625,7 @@ int idg_host_traffic_bytes(const idg_plan* plan, int direction, int64_t* h2d_byt
 
 int idg_grid_host(const idg_plan* plan, const void* vis_host, const void* aterms_host, const float* taper_host,
                   void* grid_host, void* arena_dev, size_t arena_bytes, void* cuda_stream) {
+  if (plan && plan->n_subgrids == 0) return IDG_OK;       // nothing to add: grid_host stays as it is
   if (!plan || !vis_host || !aterms_host || !taper_host || !grid_host || !arena_dev) {
     set_error("idg_grid_host: null argument");
     return IDG_EINVAL;
@@ -562,10 +635,9 @@ int idg_grid_host(const idg_plan* plan, const void* vis_host, const void* aterms
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   char* base = static_cast<char*>(arena_dev);
   const idg_params& p = plan->par;
-  const size_t L = p.subgrid_size, Ng = p.grid_size;
+  const size_t L = p.subgrid_size;
   const size_t row_b = static_cast<size_t>(p.n_chan) * 4 * sizeof(float2);
   const size_t at_b = static_cast<size_t>(p.n_stations) * plan->n_intervals * L * L * 4 * sizeof(float2);
-  const size_t grid_b = static_cast<size_t>(plan->n_wlayers) * 4 * Ng * Ng * sizeof(float2);
   const DeviceState* d = nullptr;
   int rc = ensure_device(plan, &d);
   if (rc != IDG_OK) return rc;
@@ -580,7 +652,8 @@ int idg_grid_host(const idg_plan* plan, const void* vis_host, const void* aterms
   // The caller's grid (accumulated into) is NOT on the critical path: the subgrids are added into a zeroed
   // device grid while the caller's grid goes up to a second buffer behind the visibilities, and the two are
   // summed once at the end.
-  IDG_CUDA(cudaMemsetAsync(base + a.grid, 0, grid_b, stream));
+  // (only the rows under a subgrid are zeroed, added and moved: nothing else of the device grid is ever read)
+  IDG_CUDA(for_grid_rows(plan, [&](size_t off, size_t n) { return cudaMemsetAsync(base + a.grid + off, 0, n, stream); }));
   for (size_t i = 0; i < plan->batches.size(); ++i) {
     for (const auto& run : plan->rows_first[i])
       IDG_CUDA(cudaMemcpyAsync(base + a.vis + run.first * row_b, static_cast<const char*>(vis_host) + run.first * row_b,
@@ -591,11 +664,12 @@ int idg_grid_host(const idg_plan* plan, const void* vis_host, const void* aterms
     if (rc != IDG_OK) return rc;
   }
   // only the master-grid rows under the subgrids move: the rest of grid_host is already what it will be
-  IDG_CUDA(cudaMemsetAsync(base + a.grid_in, 0, grid_b, lane.s));
   IDG_CUDA(copy_grid_rows(plan, base + a.grid_in, grid_host, cudaMemcpyHostToDevice, lane.s, nullptr));
   IDG_CUDA(lane.order(lane.s, stream));
-  IDG_CUDA(launch_grid_add(reinterpret_cast<const float2*>(base + a.grid_in), reinterpret_cast<float2*>(base + a.grid),
-                           static_cast<int64_t>(grid_b / sizeof(float2)), stream));
+  IDG_CUDA(for_grid_rows(plan, [&](size_t off, size_t n) {
+    return launch_grid_add(reinterpret_cast<const float2*>(base + a.grid_in + off), reinterpret_cast<float2*>(base + a.grid + off),
+                           static_cast<int64_t>(n / sizeof(float2)), stream);
+  }));
   IDG_CUDA(copy_grid_rows(plan, grid_host, base + a.grid, cudaMemcpyDeviceToHost, stream, nullptr));
   IDG_CUDA(cudaStreamSynchronize(stream));
   IDG_CUDA(cudaStreamSynchronize(lane.s));
@@ -604,6 +678,7 @@ int idg_grid_host(const idg_plan* plan, const void* vis_host, const void* aterms
 
 int idg_degrid_host(const idg_plan* plan, const void* grid_host, const void* aterms_host, const float* taper_host,
                     void* vis_host, void* arena_dev, size_t arena_bytes, void* cuda_stream) {
+  if (plan && plan->n_subgrids == 0) return IDG_OK;       // no planned visibility: vis_host stays as it is
   if (!plan || !vis_host || !aterms_host || !taper_host || !grid_host || !arena_dev) {
     set_error("idg_degrid_host: null argument");
     return IDG_EINVAL;
@@ -613,11 +688,10 @@ int idg_degrid_host(const idg_plan* plan, const void* grid_host, const void* ate
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   char* base = static_cast<char*>(arena_dev);
   const idg_params& p = plan->par;
-  const size_t L = p.subgrid_size, Ng = p.grid_size;
+  const size_t L = p.subgrid_size;
   const size_t row_b = static_cast<size_t>(p.n_chan) * 4 * sizeof(float2);
   const size_t vis_b = static_cast<size_t>(plan->n_rows) * row_b;
   const size_t at_b = static_cast<size_t>(p.n_stations) * plan->n_intervals * L * L * 4 * sizeof(float2);
-  const size_t grid_b = static_cast<size_t>(plan->n_wlayers) * 4 * Ng * Ng * sizeof(float2);
   const DeviceState* d = nullptr;
   int rc = ensure_device(plan, &d);
   if (rc != IDG_OK) return rc;
@@ -719,9 +793,12 @@ int idg_grid_subgrids(const idg_plan* plan, int64_t first, int64_t count, const 
   if (rc != IDG_OK) return rc;
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   const SubgridJob job = make_job(plan, d, first, count, aterms_dev, taper_dev);
-  IDG_CUDA(run_gridder(plan, job, static_cast<const float4*>(vis_dev), static_cast<float2*>(subgrids_dev), stream));
+  RangeSplit rs;
+  IDG_CUDA(rs.init(plan, first, count, IDG_GRID));
+  IDG_CUDA(run_gridder(job, rs.d, static_cast<const float4*>(vis_dev), static_cast<float2*>(subgrids_dev), stream));
   if (stage == IDG_STAGE_FFT)
     IDG_CUDA(launch_subgrid_fft(plan->par.subgrid_size, count * 4, static_cast<float2*>(subgrids_dev), +1, stream));
+  if (rs.mixed()) IDG_CUDA(cudaStreamSynchronize(stream));      // the lists are freed on return
   return IDG_OK;
 }
 
@@ -734,14 +811,86 @@ int idg_degrid_subgrids(const idg_plan* plan, int64_t first, int64_t count, cons
   int rc = ensure_device(plan, &d);
   if (rc != IDG_OK) return rc;
   const SubgridJob job = make_job(plan, d, first, count, aterms_dev, taper_dev);
-  IDG_CUDA(run_degridder(plan, job, static_cast<const float2*>(subgrids_dev), static_cast<float4*>(vis_dev),
-                            static_cast<cudaStream_t>(cuda_stream)));
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  RangeSplit rs;
+  IDG_CUDA(rs.init(plan, first, count, IDG_DEGRID));
+  IDG_CUDA(run_degridder(job, rs.d, static_cast<const float2*>(subgrids_dev), static_cast<float4*>(vis_dev), stream));
+  if (rs.mixed()) IDG_CUDA(cudaStreamSynchronize(stream));      // the lists are freed on return
+  return IDG_OK;
+}
+
+int idg_grid_subgrids_f64(const idg_plan* plan, int64_t first, int64_t count, const void* vis_dev,
+                          const void* aterms_dev, const float* taper_dev, void* subgrids_dev, void* cuda_stream) {
+  if (!plan || !vis_dev || !aterms_dev || !taper_dev || !subgrids_dev) { set_error("idg_grid_subgrids_f64: null argument"); return IDG_EINVAL; }
+  if (!range_ok(plan, first, count)) { set_error("idg_grid_subgrids_f64: bad range"); return IDG_EINVAL; }
+  if (count == 0) return IDG_OK;
+  const DeviceState* d = nullptr;
+  int rc = ensure_device(plan, &d);
+  if (rc != IDG_OK) return rc;
+  const SubgridJob job = make_job(plan, d, first, count, aterms_dev, taper_dev);
+  IDG_CUDA(launch_gridder_f64(job, static_cast<const float4*>(vis_dev), nullptr, static_cast<double2*>(subgrids_dev),
+                              static_cast<cudaStream_t>(cuda_stream)));
+  return IDG_OK;
+}
+
+int idg_degrid_subgrids_f64(const idg_plan* plan, int64_t first, int64_t count, const void* subgrids_dev,
+                            const void* aterms_dev, const float* taper_dev, void* vis_dev, void* cuda_stream) {
+  if (!plan || !vis_dev || !aterms_dev || !taper_dev || !subgrids_dev) { set_error("idg_degrid_subgrids_f64: null argument"); return IDG_EINVAL; }
+  if (!range_ok(plan, first, count)) { set_error("idg_degrid_subgrids_f64: bad range"); return IDG_EINVAL; }
+  if (count == 0) return IDG_OK;
+  const DeviceState* d = nullptr;
+  int rc = ensure_device(plan, &d);
+  if (rc != IDG_OK) return rc;
+  const SubgridJob job = make_job(plan, d, first, count, aterms_dev, taper_dev);
+  IDG_CUDA(launch_degridder_f64(job, nullptr, static_cast<const double2*>(subgrids_dev), nullptr,
+                                static_cast<double2*>(vis_dev), static_cast<cudaStream_t>(cuda_stream)));
+  return IDG_OK;
+}
+
+int idg_power_norm_average(const idg_plan* plan, const void* aterms_dev, double* avg_dev, void* cuda_stream) {
+  if (!plan || !aterms_dev || !avg_dev) { set_error("idg_power_norm_average: null argument"); return IDG_EINVAL; }
+  if (plan->n_subgrids == 0) { set_error("idg_power_norm_average: the plan has no subgrids"); return IDG_EINVAL; }
+  const DeviceState* d = nullptr;
+  int rc = ensure_device(plan, &d);
+  if (rc != IDG_OK) return rc;
+  // the factor depends on (baseline, interval) only (|| M_q M_p^H ||_F = || M_p M_q^H ||_F, so conjugated
+  // subgrids need no special case): weights = planned visibilities per (baseline, interval)
+  const int32_t n_int = plan->n_intervals;
+  std::vector<double> w(static_cast<size_t>(plan->par.n_baselines) * n_int, 0.0);
+  for (int64_t s = 0; s < plan->n_subgrids; ++s) {
+    const int32_t* e = &plan->sub[static_cast<size_t>(s) * 8];
+    w[static_cast<size_t>(e[0]) * n_int + e[1] / plan->par.aterm_period] += static_cast<double>(e[2]) * e[4];
+  }
+  std::vector<int32_t> pairs;
+  std::vector<double> weights;
+  double wsum = 0.0;
+  for (size_t i = 0; i < w.size(); ++i) {
+    if (w[i] == 0.0) continue;
+    const size_t b = i / n_int;
+    pairs.push_back(plan->baselines[b * 2]); pairs.push_back(plan->baselines[b * 2 + 1]);
+    pairs.push_back(static_cast<int32_t>(i % n_int));
+    weights.push_back(w[i]);
+    wsum += w[i];
+  }
+  const int L = plan->par.subgrid_size;
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  int32_t* d_pairs = nullptr;
+  double *d_w = nullptr, *d_scratch = nullptr;
+  cudaError_t e = upload(pairs, &d_pairs);
+  if (e == cudaSuccess) e = upload(weights, &d_w);
+  if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&d_scratch), sizeof(double) * kPowerNormSlices * L * L);
+  if (e == cudaSuccess)
+    e = launch_power_norm_average(static_cast<const float4*>(aterms_dev), L, n_int, d_pairs, d_w,
+                                  static_cast<int64_t>(weights.size()), wsum, d_scratch, avg_dev, stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+  cudaFree(d_pairs); cudaFree(d_w); cudaFree(d_scratch);
+  if (e != cudaSuccess) return cuda_fail(e, "idg_power_norm_average");
   return IDG_OK;
 }
 
 int idg_subgrid_fft(int32_t subgrid_size, int64_t n_planes, void* planes_dev, int direction, void* cuda_stream) {
-  if (subgrid_size != 32 && subgrid_size != 64 && subgrid_size != 96 && subgrid_size != 128) {
-    set_error("idg_subgrid_fft: subgrid_size must be 32, 64, 96 or 128");
+  if (!subgrid_size_ok(subgrid_size)) {
+    set_error("idg_subgrid_fft: subgrid_size must be 32, 48, 64, 96, 128 or 160");
     return IDG_EUNSUPPORTED;
   }
   if (n_planes < 0 || (n_planes > 0 && !planes_dev) || (direction != 1 && direction != -1)) {
@@ -819,19 +968,9 @@ int idg_profile_read(double* ms_out, int64_t* launches_out) {
   return IDG_OK;
 }
 
-int idg_set_kernel_variant(int kind, int variant) {
-  if ((kind != IDG_K_GRIDDER && kind != IDG_K_DEGRIDDER) ||
-      (variant != IDG_VARIANT_SIMT && variant != IDG_VARIANT_TENSOR && variant != IDG_VARIANT_AUTO)) {
-    set_error("idg_set_kernel_variant: bad kind or variant");
-    return IDG_EINVAL;
-  }
-  g_variant[kind].store(variant);
-  return IDG_OK;
-}
-
-int idg_get_kernel_variant(int kind) {
-  if (kind < 0 || kind >= IDG_K_COUNT) return IDG_EINVAL;
-  return g_variant[kind].load();
+int idg_kernel_config_mask(int kind, int reset) {
+  if (kind != IDG_K_GRIDDER && kind != IDG_K_DEGRIDDER) { set_error("idg_kernel_config_mask: bad kind"); return IDG_EINVAL; }
+  return reset ? g_kmask[kind].exchange(0) : g_kmask[kind].load();
 }
 
 int idg_measure_alu_peaks(double* out_host) {

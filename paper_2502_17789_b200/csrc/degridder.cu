@@ -30,14 +30,18 @@ __global__ void __launch_bounds__(T) degridder_kernel(const SubgridJob job, cons
   constexpr int NSEG = kPixChunk / kSeg;
   constexpr int NCHUNK = L * L / kPixChunk;
 
-  __shared__ __align__(16) float4 spix[kPixChunk][5];   // 4 x (re,re,im,im) + (n', n', fx, fx)
+  __shared__ __align__(16) float4 spix[kPixChunk][5];   // 4 x (re,re,im,im) + (n', n', fx, fx), fx within the segment
   __shared__ __align__(16) float4 sred[T][2];
 
   const int tid = threadIdx.x, warp = tid / 32, lane = tid % 32;
-  const int sg = blockIdx.x;
+  const int64_t sg = job_slot(job, blockIdx.x);
   const int32_t* __restrict__ m = job.meta + (job.first + sg) * kMetaStride;
   const int b = m[0], t0 = m[1], nt = m[2], c0 = m[3], nc = m[4], x0 = m[5], y0 = m[6], wl = m[7];
   const int sp = m[8], sq = m[9], it = m[10];
+  // rows used as (-u,-v,-w) of the swapped baseline: the sum predicts V(-u,-v,-w) of (q,p) and its dagger is
+  // written (PAPER.md:178 fn 4, R21)
+  const bool conj = (m[12] & kMetaConj) != 0;
+  const double sgn = conj ? -1.0 : 1.0;
 
   const double S = job.image_size;
   const double u0 = (x0 + L / 2 - job.grid_size / 2) / S;
@@ -47,7 +51,7 @@ __global__ void __launch_bounds__(T) degridder_kernel(const SubgridJob job, cons
 
   const float4* __restrict__ ap = job.aterms + (static_cast<int64_t>(sp) * job.n_intervals + it) * (L * L * 2);
   const float4* __restrict__ aq = job.aterms + (static_cast<int64_t>(sq) * job.n_intervals + it) * (L * L * 2);
-  const float2* __restrict__ sub = in + static_cast<int64_t>(sg) * 4 * L * L;
+  const float2* __restrict__ sub = in + sg * 4 * L * L;
 
   const int K = nt * nc;
   const int n_vt = (K + PV - 1) / PV;        // visibility-threads needed
@@ -60,22 +64,29 @@ __global__ void __launch_bounds__(T) degridder_kernel(const SubgridJob job, cons
   for (int vb = 0; vb < VW; vb += VWB) {
     const int v = (vb + vw) * 32 + lane;
     // my PV visibilities: k_j = j * n_vt + v  (consecutive lanes -> consecutive visibilities)
-    float2 al[PV / 2], be[PV / 2], ga[PV / 2];
+    // phase [rad] = al fx + be fy + ga n'.  The part linear in the pixel position reaches hundreds of radians at
+    // the subgrid's edge, so the first pixel of every 16-pixel segment takes it modulo one cycle EXACTLY in 32-bit
+    // fixed point (afix * ix + bfix * iy wraps), as the gridders do; al * (0..15) and ga n' are fp32.
+    float2 al[PV / 2], ga[PV / 2];
+    int32_t afix[PV], bfix[PV];                  // cycles per pixel * 2^32
 #pragma unroll
     for (int j = 0; j < PV; ++j) {
       const int k = j * n_vt + v;
-      float a_ = 0.f, b_ = 0.f, g_ = 0.f;
+      float a_ = 0.f, g_ = 0.f;
+      afix[j] = bfix[j] = 0;
       if (active && v < n_vt && k < K) {
         const int r = k / nc, c = k % nc;
         const double* uvw = job.uvw + (row0 + r) * 3;
         const double kap = job.kappa[c0 + c];
         const double two_pi = 6.283185307179586476925286766559;
-        a_ = static_cast<float>(two_pi * ((uvw[0] * kap - u0) * (S / L)));
-        b_ = static_cast<float>(two_pi * ((uvw[1] * kap - v0) * (S / L)));
-        g_ = static_cast<float>(two_pi * (uvw[2] * kap - w0));
+        const double alpha = (sgn * uvw[0] * kap - u0) * (S / L), beta = (sgn * uvw[1] * kap - v0) * (S / L);
+        a_ = static_cast<float>(two_pi * alpha);
+        afix[j] = static_cast<int32_t>(static_cast<uint32_t>(static_cast<int64_t>(rint(alpha * 4294967296.0))));
+        bfix[j] = static_cast<int32_t>(static_cast<uint32_t>(static_cast<int64_t>(rint(beta * 4294967296.0))));
+        g_ = static_cast<float>(two_pi * (sgn * uvw[2] * kap - w0));
       }
-      if (j & 1) { al[j / 2].y = a_; be[j / 2].y = b_; ga[j / 2].y = g_; }
-      else       { al[j / 2].x = a_; be[j / 2].x = b_; ga[j / 2].x = g_; }
+      if (j & 1) { al[j / 2].y = a_; ga[j / 2].y = g_; }
+      else       { al[j / 2].x = a_; ga[j / 2].x = g_; }
     }
     float2 vre[4][PV / 2], vim[4][PV / 2];
 #pragma unroll
@@ -99,17 +110,19 @@ __global__ void __launch_bounds__(T) degridder_kernel(const SubgridJob job, cons
 #pragma unroll
         for (int p = 0; p < 4; ++p) spix[i][p] = make_float4(z[p].x, z[p].x, z[p].y, z[p].y);
         const float np = __ldg(&job.nprime[pix]);
-        const float fx = static_cast<float>(pix % L - L / 2);
+        const float fx = static_cast<float>(i % kSeg);    // offset within the 16-pixel segment
         spix[i][4] = make_float4(np, np, fx, fx);
       }
       __syncthreads();
       if (active) {
         for (int seg = g; seg < NSEG; seg += G) {
           const int q0 = chunk * kPixChunk + seg * kSeg;
-          const float fy = static_cast<float>(q0 / L - L / 2);
+          const int ix0 = q0 % L - L / 2, iy = q0 / L - L / 2;
           float2 tt[PV / 2];
 #pragma unroll
-          for (int j = 0; j < PV / 2; ++j) tt[j] = make_float2(be[j].x * fy, be[j].y * fy);
+          for (int j = 0; j < PV / 2; ++j)
+            tt[j] = make_float2(static_cast<float>(afix[2 * j] * ix0 + bfix[2 * j] * iy) * 1.4629180792671596e-9f,
+                                static_cast<float>(afix[2 * j + 1] * ix0 + bfix[2 * j + 1] * iy) * 1.4629180792671596e-9f);
 #pragma unroll 2
           for (int i = 0; i < kSeg; ++i) {
             const float4* rec = spix[seg * kSeg + i];
@@ -157,6 +170,10 @@ __global__ void __launch_bounds__(T) degridder_kernel(const SubgridJob job, cons
         }
         const int r = k / nc, c = k % nc;
         float4* o = vis + ((row0 + r) * job.n_chan + c0 + c) * 2;
+        if (conj) {                                     // (XX, XY, YX, YY) <- conj of (XX, YX, XY, YY)
+          const float4 d0 = make_float4(a0.x, -a0.y, a1.x, -a1.y), d1 = make_float4(a0.z, -a0.w, a1.z, -a1.w);
+          a0 = d0; a1 = d1;
+        }
         o[0] = a0;
         o[1] = a1;
       }
@@ -169,6 +186,7 @@ cudaError_t launch(const SubgridJob& job, const float2* in, float4* vis, cudaStr
   if (job.count == 0) return cudaSuccess;
   degridder_kernel<L, T, PV><<<static_cast<unsigned>(job.count), T, 0, stream>>>(job, in, vis);
   count_launch();
+  note_kernel(IDG_K_DEGRIDDER, IDG_KMASK_SIMT);
   return cudaGetLastError();
 }
 
@@ -177,9 +195,11 @@ cudaError_t launch(const SubgridJob& job, const float2* in, float4* vis, cudaStr
 cudaError_t launch_degridder(const SubgridJob& job, const float2* in, float4* vis, cudaStream_t stream) {
   switch (job.subgrid_size) {
     case 32:  return launch<32, 256, 8>(job, in, vis, stream);
+    case 48:  return launch<48, 256, 8>(job, in, vis, stream);
     case 64:  return launch<64, 256, 8>(job, in, vis, stream);
     case 96:  return launch<96, 256, 8>(job, in, vis, stream);
     case 128: return launch<128, 256, 8>(job, in, vis, stream);
+    case 160: return launch<160, 256, 8>(job, in, vis, stream);
     default:  return cudaErrorInvalidValue;
   }
 }

@@ -25,6 +25,7 @@
 //                    (M = 128, N = 16, K = 8) per chunk, commits to empty[slot], to dfull at an
 //                    accumulator group's end and to the stage's empty barrier after its last chunk.
 #include <algorithm>
+#include <type_traits>
 
 #include "device_math.cuh"
 #include "kernels.h"
@@ -88,10 +89,13 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
   __shared__ uint32_t s_tmem;
 
   const int tid = threadIdx.x, warp = tid / 32, lane = tid % 32;
-  const int64_t sg = blockIdx.x;
+  const int64_t sg = job_slot(job, blockIdx.x);
   const int32_t* m = job.meta + (job.first + sg) * kMetaStride;
   const int b = m[0], t0 = m[1], nt = m[2], c0 = m[3], nc = m[4], x0 = m[5], y0 = m[6], wl = m[7];
   const int sp = m[8], sq = m[9], it = m[10];
+  // rows used as (-u,-v,-w) of the swapped baseline: the sum predicts V(-u,-v,-w) of (q,p) and its dagger is
+  // written (PAPER.md:178 fn 4, R21)
+  const bool conj = (m[12] & kMetaConj) != 0;
   const int64_t row0 = static_cast<int64_t>(b) * job.n_times + t0;
   const int K = nt * nc;                               // visibilities of the subgrid
   const int T = (K + kTileV - 1) / kTileV;             // visibility tiles
@@ -249,8 +253,13 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
 
     if (is_compute && active) {
       // ===== compute threads: one visibility of the group's tile each =====
-      // phase [rad] = al fx + be fy + ga n', offsets relative to the subgrid centre from fp64
-      float al = 0.f, be = 0.f, ga = 0.f;
+      // phase [rad] = al fx + be fy + ga n', offsets relative to the subgrid centre from fp64.  The part that is
+      // linear in the pixel position reaches hundreds of radians at the subgrid's edge (L = 128, 160), more than
+      // fp32 resolves to 1e-6, so a chunk's first pixel takes it modulo one cycle EXACTLY, in 32-bit fixed
+      // point (alpha_fix * ix + beta_fix * iy wraps), as the gridders do; only al * j (j < 8) and ga n' are fp32.
+      float al = 0.f, ga = 0.f;
+      [[maybe_unused]] float be_f = 0.f;
+      int32_t alpha_fix = 0, beta_fix = 0;             // cycles per pixel * 2^32
       if (vis_ok) {
         const double S = job.image_size;
         const double u0 = (x0 + L / 2 - job.grid_size / 2) / S;
@@ -259,10 +268,21 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
         const double* uvw = job.uvw + (row0 + vr) * 3;
         const double kap = job.kappa[c0 + vc];
         const double two_pi = 6.283185307179586476925286766559;
-        al = static_cast<float>(two_pi * ((uvw[0] * kap - u0) * (S / L)));
-        be = static_cast<float>(two_pi * ((uvw[1] * kap - v0) * (S / L)));
-        ga = static_cast<float>(two_pi * (uvw[2] * kap - w0));
+        const double sgn = conj ? -1.0 : 1.0;
+        const double alpha = (sgn * uvw[0] * kap - u0) * (S / L), beta = (sgn * uvw[1] * kap - v0) * (S / L);
+        al = static_cast<float>(two_pi * alpha);
+#ifdef IDG_DTC_FLOATBASE
+        be_f = static_cast<float>(two_pi * beta);
+#endif
+        alpha_fix = static_cast<int32_t>(static_cast<uint32_t>(static_cast<int64_t>(rint(alpha * 4294967296.0))));
+        beta_fix = static_cast<int32_t>(static_cast<uint32_t>(static_cast<int64_t>(rint(beta * 4294967296.0))));
+        ga = static_cast<float>(two_pi * (sgn * uvw[2] * kap - w0));
       }
+      // A warp none of whose 32 visibilities exists (the ragged tail of the subgrid's last tile) generates no
+      // phasors and stores nothing: it only keeps the ring's barriers in step (its tensor-memory rows hold
+      // stale finite-or-not values that no thread reads: MMA rows are independent).  The SIMT work is thus
+      // padded to 32 visibilities, not 128 (low-occupancy tails).
+      const bool warp_on = (t_base + tile_l) * kTileV + (uwarp & 3) * 32 < K;      // from warp-uniform values only
       bool pending = false;                            // the ring's last slot is stored but not yet handed over
       auto drain = [&](int qq) {
         tc::mbar_wait(gbar + 16 * NA + 8 * (qq & 1), (qq >> 1) & 1);
@@ -283,17 +303,21 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
 
       const uint32_t snp_addr = tc::smem_u32(snp);
       uint32_t np_addr = 0;                            // n' of the next chunk's pixels
-      float fx0 = 0.f, fy = 0.f;                       // pixel offsets of the next chunk's first pixel
+      int ix0 = 0, iy = 0;                             // pixel offsets of the next chunk's first pixel
       // cl = chunks left in my share of the current stage; kept in plain registers (`opaque`)
       const int ncs_r = static_cast<int>(tc::opaque(static_cast<uint32_t>(ncs)));
       const int lp0 = static_cast<int>(tc::opaque(static_cast<uint32_t>((part << lgn) * kKC)));
       int cl = 0, st = 0, rig = 0, gin = 0;
+      // the round's chunk loop, in two copies: warps with visibilities (ON: no test inside the loop) and the
+      // bookkeeping-only copy for the warps of a ragged tail
+      auto chunk_loop = [&](auto on_tag) {
+      constexpr bool ON = decltype(on_tag)::value;
       for (int rev = 0; rev < nrev; ++rev) {
 #pragma unroll
         for (int s = 0; s < NA; ++s) {
           // slots past the round's last chunk are computed and stored like any other (the service warp issues
           // no MMA for them), so the compute threads never test whether a slot is in use
-          constexpr bool valid = true;
+          constexpr bool valid = ON;
           // the previous slot goes to the service warp before this one's arithmetic
           if (s > 0) hand_off(gbar + 8 * (s - 1));
           else if (pending) hand_off(gbar + 8 * (NA - 1));
@@ -305,15 +329,19 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
               tc::mbar_wait(bar_sfull + 8 * slot, (gst / NS) & 1);
               const int pix0 = st * kStagePix + lp0;
               np_addr = snp_addr + (slot * kStagePix + lp0) * 4;
-              fx0 = static_cast<float>(pix0 % L - L / 2);
-              fy = static_cast<float>(pix0 / L - L / 2);
+              ix0 = pix0 % L - L / 2;
+              iy = pix0 / L - L / 2;
               ++st;
               cl = ncs_r;
             }
             const float4 na = tc::lds128(np_addr), nb = tc::lds128(np_addr + 16);
             const float2 np2[4] = {make_float2(na.x, na.y), make_float2(na.z, na.w),
                                    make_float2(nb.x, nb.y), make_float2(nb.z, nb.w)};
-            const float base = fmaf(al, fx0, be * fy);
+#ifdef IDG_DTC_FLOATBASE
+            const float base = fmaf(al, static_cast<float>(ix0), be_f * static_cast<float>(iy));
+#else
+            const float base = static_cast<float>(alpha_fix * ix0 + beta_fix * iy) * 1.4629180792671596e-9f;   // 2 pi / 2^32
+#endif
             const float2 base2 = make_float2(base, base), al2 = make_float2(al, al), ga2 = make_float2(ga, ga);
             const float2 m1 = make_float2(-1.f, -1.f);
 #pragma unroll
@@ -342,8 +370,8 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
             tc::tmem_st16(gtmem + s * A_COLS, hi);
             tc::tmem_st16(gtmem + s * A_COLS + 2 * kKC, lo);
             np_addr += kKC * 4;
-            fx0 += static_cast<float>(kKC);
-            if (fx0 >= static_cast<float>(L / 2)) { fx0 = static_cast<float>(-L / 2); fy += 1.f; }
+            ix0 += kKC;
+            if (ix0 >= L / 2) { ix0 = -L / 2; ++iy; }
             --cl;
           }
         }
@@ -355,6 +383,8 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
           rig = 0; ++q; ++gin;
         }
       }
+      };
+      if (warp_on) chunk_loop(std::true_type{}); else chunk_loop(std::false_type{});
       hand_off(gbar + 8 * (NA - 1));
       drain(q - 1);
       // partial sums of the groups that share my tile meet in shared memory
@@ -373,8 +403,13 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
         acc[4] += a1.x; acc[5] += a1.y; acc[6] += a1.z; acc[7] += a1.w;
       }
       float4* o = vis + ((row0 + vr) * job.n_chan + c0 + vc) * 2;
-      o[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
-      o[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
+      if (conj) {                                       // (XX, XY, YX, YY) <- conj of (XX, YX, XY, YY)
+        o[0] = make_float4(acc[0], -acc[1], acc[4], -acc[5]);
+        o[1] = make_float4(acc[2], -acc[3], acc[6], -acc[7]);
+      } else {
+        o[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
+        o[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
+      }
     }
     __syncthreads();
   }
@@ -393,14 +428,12 @@ cudaError_t launch(const SubgridJob& job, const float2* in, float4* vis, cudaStr
   constexpr int NG = IDG_DTC_NG, NS = NG == 2 ? 2 : IDG_DTC_NS;
   constexpr size_t dyn = NS * kStageBBytes + NS * kStagePix * 4 + (NG - 1) * kTileV * 8 * 4;
   auto kernel = degridder_tc_kernel<L, NG, IDG_DTC_DG, IDG_DTC_NA, NS>;
-  static bool configured = false;                      // per instantiation
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn));
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  // per launch: the attribute belongs to the (function, device) pair and the call is cheap
+  cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn));
+  if (e != cudaSuccess) return e;
   kernel<<<static_cast<unsigned>(job.count), NG * kTileV + NG * 32 + kProducers * 32, dyn, stream>>>(job, in, vis);
   count_launch();
+  note_kernel(IDG_K_DEGRIDDER, IDG_KMASK_TC(NG));
   return cudaGetLastError();
 }
 
@@ -409,9 +442,11 @@ cudaError_t launch(const SubgridJob& job, const float2* in, float4* vis, cudaStr
 cudaError_t launch_degridder_tc(const SubgridJob& job, const float2* in, float4* vis, cudaStream_t stream) {
   switch (job.subgrid_size) {
     case 32:  return launch<32>(job, in, vis, stream);
+    case 48:  return launch<48>(job, in, vis, stream);
     case 64:  return launch<64>(job, in, vis, stream);
     case 96:  return launch<96>(job, in, vis, stream);
     case 128: return launch<128>(job, in, vis, stream);
+    case 160: return launch<160>(job, in, vis, stream);
     default:  return cudaErrorInvalidValue;
   }
 }

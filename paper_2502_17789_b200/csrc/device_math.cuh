@@ -32,6 +32,21 @@ __device__ __forceinline__ void sandwich(const float2 x[4], float4 mp0, float4 m
   r = cadd(cmulc(y10, q10), cmulc(y11, q11)); z[3] = make_float2(t * r.x, t * r.y);
 }
 
+// 1 / || Mp Mq^H ||_F of row-major 2x2 complex matrices (section 3.3, R22): the power
+// normalisation of the imaging sandwich.  IEEE sqrt and division (no fast-math approximations).
+__device__ __forceinline__ float frobenius_inv(float4 mp0, float4 mp1, float4 mq0, float4 mq1) {
+  const float2 a = make_float2(mp0.x, mp0.y), b = make_float2(mp0.z, mp0.w);
+  const float2 c = make_float2(mp1.x, mp1.y), d = make_float2(mp1.z, mp1.w);
+  const float2 q00 = make_float2(mq0.x, mq0.y), q01 = make_float2(mq0.z, mq0.w);
+  const float2 q10 = make_float2(mq1.x, mq1.y), q11 = make_float2(mq1.z, mq1.w);
+  // (Mp Mq^H)[i][j] = sum_k Mp[i][k] conj(Mq[j][k])
+  const float2 p00 = cadd(cmulc(a, q00), cmulc(b, q01)), p01 = cadd(cmulc(a, q10), cmulc(b, q11));
+  const float2 p10 = cadd(cmulc(c, q00), cmulc(d, q01)), p11 = cadd(cmulc(c, q10), cmulc(d, q11));
+  const float n2 = (p00.x * p00.x + p00.y * p00.y) + (p01.x * p01.x + p01.y * p01.y) +
+                   (p10.x * p10.x + p10.y * p10.y) + (p11.x * p11.x + p11.y * p11.y);
+  return __fdiv_rn(1.f, __fsqrt_rn(n2));
+}
+
 __device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
 __device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
 

@@ -5,7 +5,8 @@
 // output), so the kernel is a plain 2-D FFT with the checkerboard folded into the global load and
 // the checkerboard and 1/L^2 into the global store.
 //
-// Every 1-D transform of length L = 8 R2 (R2 = 4, 8, 12, 16) is two register-resident steps:
+// Every 1-D transform of length L = 8 R2 (R2 = 4, 6, 8, 12, 16, 20: L = 32, 48, 64, 96, 128, 160, the range of
+// PAPER.md Fig. 7 :363-369) is two register-resident steps:
 //   n = n1 R2 + n2, k = k1 + 8 k2:
 //   step 1  Y[k1][n2] = w_L^(n2 k1) * sum_n1 x[n1 R2 + n2] w_8^(n1 k1)     (radix-8 butterfly per n2)
 //   step 2  X[k1 + 8 k2] = sum_n2 Y[k1][n2] w_R2^(n2 k2)                   (radix-R2 butterfly per k1)
@@ -36,6 +37,19 @@ __device__ __forceinline__ float2 wsmall(int m) {
   if constexpr (N == 8) {
     const float c[8] = {1.f, 0.707106781f, 0.f, -0.707106781f, -1.f, -0.707106781f, 0.f, 0.707106781f};
     const float s[8] = {0.f, 0.707106781f, 1.f, 0.707106781f, 0.f, -0.707106781f, -1.f, -0.707106781f};
+    return make_float2(c[m], SIGN * s[m]);
+  } else if constexpr (N == 6) {
+    const float c[6] = {1.f, 0.5f, -0.5f, -1.f, -0.5f, 0.5f};
+    const float s[6] = {0.f, 0.866025404f, 0.866025404f, 0.f, -0.866025404f, -0.866025404f};
+    return make_float2(c[m], SIGN * s[m]);
+  } else if constexpr (N == 20) {
+    const float c[20] = {1.f, 0.951056516f, 0.809016994f, 0.587785252f, 0.309016994f, 0.f, -0.309016994f,
+                         -0.587785252f, -0.809016994f, -0.951056516f, -1.f, -0.951056516f, -0.809016994f,
+                         -0.587785252f, -0.309016994f, 0.f, 0.309016994f, 0.587785252f, 0.809016994f, 0.951056516f};
+    const float s[20] = {0.f, 0.309016994f, 0.587785252f, 0.809016994f, 0.951056516f, 1.f, 0.951056516f,
+                         0.809016994f, 0.587785252f, 0.309016994f, 0.f, -0.309016994f, -0.587785252f,
+                         -0.809016994f, -0.951056516f, -1.f, -0.951056516f, -0.809016994f, -0.587785252f,
+                         -0.309016994f};
     return make_float2(c[m], SIGN * s[m]);
   } else if constexpr (N == 12) {
     const float c[12] = {1.f, 0.866025404f, 0.5f, 0.f, -0.5f, -0.866025404f, -1.f, -0.866025404f, -0.5f, 0.f, 0.5f,
@@ -73,13 +87,43 @@ __device__ __forceinline__ void dft4(float2& x0, float2& x1, float2& x2, float2&
   const float2 a = cadd2(x0, x2), b = csub2(x0, x2), c = cadd2(x1, x3), d = rot90<SIGN>(csub2(x1, x3));
   x0 = cadd2(a, c); x1 = cadd2(b, d); x2 = csub2(a, c); x3 = csub2(b, d);
 }
+// X[k] = sum x[n] w^(nk), w = exp(SIGN 2 pi i / 5): conjugate pairs (1, 4) and (2, 3)
+template <int SIGN>
+__device__ __forceinline__ void dft5(float2& x0, float2& x1, float2& x2, float2& x3, float2& x4) {
+  const float c1 = 0.30901699437494742410f, c2 = -0.80901699437494742410f;          // cos 2 pi/5, cos 4 pi/5
+  const float s1 = SIGN * 0.95105651629515357212f, s2 = SIGN * 0.58778525229247312917f;   // sin 2 pi/5, sin 4 pi/5
+  const float2 p1 = cadd2(x1, x4), d1 = csub2(x1, x4), p2 = cadd2(x2, x3), d2 = csub2(x2, x3);
+  const float2 a1 = make_float2(fmaf(c1, p1.x, fmaf(c2, p2.x, x0.x)), fmaf(c1, p1.y, fmaf(c2, p2.y, x0.y)));
+  const float2 a2 = make_float2(fmaf(c2, p1.x, fmaf(c1, p2.x, x0.x)), fmaf(c2, p1.y, fmaf(c1, p2.y, x0.y)));
+  const float2 e1 = make_float2(fmaf(s1, d1.x, s2 * d2.x), fmaf(s1, d1.y, s2 * d2.y));   // then times i
+  const float2 e2 = make_float2(fmaf(s2, d1.x, -s1 * d2.x), fmaf(s2, d1.y, -s1 * d2.y));
+  const float2 b1 = make_float2(-e1.y, e1.x), b2 = make_float2(-e2.y, e2.x);
+  x0 = cadd2(x0, cadd2(p1, p2));
+  x1 = cadd2(a1, b1); x4 = csub2(a1, b1);
+  x2 = cadd2(a2, b2); x3 = csub2(a2, b2);
+}
 // N = P Q by the same index split as above: n = n1 Q + n2, k = k1 + P k2
 template <int N, int SIGN>
 __device__ __forceinline__ void dft_small(float2 (&x)[N]) {
   if constexpr (N == 4) {
     dft4<SIGN>(x[0], x[1], x[2], x[3]);
+  } else if constexpr (N == 6) {                     // 6 = 2 x 3
+    float2 y[6];                                     // y[k1 * 3 + n2]
+#pragma unroll
+    for (int n2 = 0; n2 < 3; ++n2) {
+      float2 a = x[n2], b = x[3 + n2];
+      dft2<SIGN>(a, b);
+      y[n2] = a;
+      y[3 + n2] = n2 ? cmulf(b, wsmall<6, SIGN>(n2)) : b;
+    }
+#pragma unroll
+    for (int k1 = 0; k1 < 2; ++k1) {
+      dft3<SIGN>(y[k1 * 3], y[k1 * 3 + 1], y[k1 * 3 + 2]);
+#pragma unroll
+      for (int k2 = 0; k2 < 3; ++k2) x[k1 + 2 * k2] = y[k1 * 3 + k2];
+    }
   } else {
-    constexpr int P = 4, Q = N / 4;                  // 8 = 4 x 2, 12 = 4 x 3, 16 = 4 x 4
+    constexpr int P = 4, Q = N / 4;                  // 8 = 4 x 2, 12 = 4 x 3, 16 = 4 x 4, 20 = 4 x 5
     float2 y[N];                                     // y[k1 * Q + n2]
 #pragma unroll
     for (int n2 = 0; n2 < Q; ++n2) {
@@ -96,6 +140,8 @@ __device__ __forceinline__ void dft_small(float2 (&x)[N]) {
         dft2<SIGN>(y[k1 * Q], y[k1 * Q + 1]);
       } else if constexpr (Q == 3) {
         dft3<SIGN>(y[k1 * Q], y[k1 * Q + 1], y[k1 * Q + 2]);
+      } else if constexpr (Q == 5) {
+        dft5<SIGN>(y[k1 * Q], y[k1 * Q + 1], y[k1 * Q + 2], y[k1 * Q + 3], y[k1 * Q + 4]);
       } else {
         dft4<SIGN>(y[k1 * Q], y[k1 * Q + 1], y[k1 * Q + 2], y[k1 * Q + 3]);
       }
@@ -106,7 +152,9 @@ __device__ __forceinline__ void dft_small(float2 (&x)[N]) {
 }
 
 template <int L>
-struct FftThreads { static constexpr int value = L == 32 ? 128 : (L == 64 ? 256 : (L == 96 ? 576 : 512)); };
+struct FftThreads {
+  static constexpr int value = L == 32 ? 128 : (L == 48 ? 192 : (L == 64 ? 256 : (L == 96 ? 576 : (L == 128 ? 512 : 640))));
+};
 
 // Where the transform reads its input: the plane itself (in place), or, for the prediction direction, the
 // master grid patch under the subgrid (step a6, the splitter, fused into the load of step a7).
@@ -123,7 +171,7 @@ __global__ void __launch_bounds__(FftThreads<L>::value) fft_kernel(float2* __res
   // Row step 1 stores 8 groups of R2 + 1.  With the pitch = 8 (mod 16) float2, the 4 rows a warp touches in
   // the row steps land on complementary halves of the 16 8-byte bank slots: every access is conflict-free.
   constexpr int PITCH = L + 8;
-  static_assert(R2 == 4 || R2 == 8 || R2 == 12 || R2 == 16, "L = 8 R2");
+  static_assert(R2 == 4 || R2 == 6 || R2 == 8 || R2 == 12 || R2 == 16 || R2 == 20, "L = 8 R2, R2 even");
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float2* data = reinterpret_cast<float2*>(smem_raw);          // [L][PITCH]
   float2* tw = data + L * PITCH;                               // [L] exp(SIGN 2 pi i m / L)
@@ -256,9 +304,11 @@ cudaError_t launch_subgrid_fft(int L, int64_t n_planes, float2* planes, int dire
   const GridSource none{nullptr, nullptr, 0};
   switch (L) {
     case 32:  return launch<32>(n_planes, planes, direction, none, stream);
+    case 48:  return launch<48>(n_planes, planes, direction, none, stream);
     case 64:  return launch<64>(n_planes, planes, direction, none, stream);
     case 96:  return launch<96>(n_planes, planes, direction, none, stream);
     case 128: return launch<128>(n_planes, planes, direction, none, stream);
+    case 160: return launch<160>(n_planes, planes, direction, none, stream);
     default:  return cudaErrorInvalidValue;
   }
 }
@@ -268,9 +318,11 @@ cudaError_t launch_split_ifft(const int32_t* meta, int64_t first, int64_t count,
   const GridSource src{grid, meta + first * kMetaStride, Ng};
   switch (L) {
     case 32:  return launch<32>(count * 4, subgrids, -1, src, stream);
+    case 48:  return launch<48>(count * 4, subgrids, -1, src, stream);
     case 64:  return launch<64>(count * 4, subgrids, -1, src, stream);
     case 96:  return launch<96>(count * 4, subgrids, -1, src, stream);
     case 128: return launch<128>(count * 4, subgrids, -1, src, stream);
+    case 160: return launch<160>(count * 4, subgrids, -1, src, stream);
     default:  return cudaErrorInvalidValue;
   }
 }

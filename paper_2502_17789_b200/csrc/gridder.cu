@@ -44,11 +44,12 @@ __global__ void __launch_bounds__(T) gridder_kernel(const SubgridJob job, const 
   __shared__ RowData srow[2];
 
   const int tid = threadIdx.x;
-  const int sg = blockIdx.x / PIECES;
+  const int64_t sg = job_slot(job, blockIdx.x / PIECES);
   const int piece = blockIdx.x % PIECES;
   const int32_t* __restrict__ m = job.meta + (job.first + sg) * kMetaStride;
   const int b = m[0], t0 = m[1], nt = m[2], c0 = m[3], nc = m[4], x0 = m[5], y0 = m[6], wl = m[7];
   const int sp = m[8], sq = m[9], it = m[10];
+  const bool conj = (m[12] & kMetaConj) != 0;          // rows used as (-u,-v,-w) with V^dagger (PAPER.md:178 fn 4, R21)
 
   const double S = job.image_size;
   const double u0 = (x0 + L / 2 - job.grid_size / 2) / S;
@@ -80,7 +81,14 @@ __global__ void __launch_bounds__(T) gridder_kernel(const SubgridJob job, const 
     const int r = ci / cpr, cc = (ci % cpr) * kChunk;
     const int cnt = min(kChunk, nc - cc);
     if (tid < 2 * cnt) {
-      pre = __ldg(&vis[((row0 + r) * job.n_chan + c0 + cc) * 2 + tid]);
+      if (!conj) {
+        pre = __ldg(&vis[((row0 + r) * job.n_chan + c0 + cc) * 2 + tid]);
+      } else {
+        // V^dagger = conj of (XX, YX, XY, YY): this thread's pair is (XX, YX)* or (XY, YY)*
+        const float2* v2 = reinterpret_cast<const float2*>(vis) + ((row0 + r) * job.n_chan + c0 + cc + (tid >> 1)) * 4;
+        const float2 a = __ldg(&v2[tid & 1]), b2 = __ldg(&v2[2 + (tid & 1)]);
+        pre = make_float4(a.x, -a.y, b2.x, -b2.y);
+      }
       if (job.weights != nullptr) {                     // weighting at load
         const float wgt = __ldg(&job.weights[(row0 + r) * job.n_chan + c0 + cc + (tid >> 1)]);
         pre = make_float4(pre.x * wgt, pre.y * wgt, pre.z * wgt, pre.w * wgt);
@@ -98,7 +106,8 @@ __global__ void __launch_bounds__(T) gridder_kernel(const SubgridJob job, const 
     if (tid < cnt) sdk[buf][tid] = static_cast<float>(job.kappa[c0 + cc + tid] - kref);
     if (tid == T - 1) {
       const double* uvw = job.uvw + (row0 + r) * 3;
-      const double um = uvw[0], vm = uvw[1], wm = uvw[2];
+      const double sgn = conj ? -1.0 : 1.0;
+      const double um = sgn * uvw[0], vm = sgn * uvw[1], wm = sgn * uvw[2];
       const double two_pi = 6.283185307179586476925286766559;
       const double sl = S / L;
       const double alpha = (um * kref - u0) * sl, beta = (vm * kref - v0) * sl;
@@ -167,7 +176,7 @@ __global__ void __launch_bounds__(T) gridder_kernel(const SubgridJob job, const 
   // --- epilogue (step a3): A-term sandwich and taper, once per pixel.
   const float4* __restrict__ ap = job.aterms + (static_cast<int64_t>(sp) * job.n_intervals + it) * (L * L * 2);
   const float4* __restrict__ aq = job.aterms + (static_cast<int64_t>(sq) * job.n_intervals + it) * (L * L * 2);
-  float2* __restrict__ o = out + static_cast<int64_t>(sg) * 4 * L * L;
+  float2* __restrict__ o = out + sg * 4 * L * L;
 #pragma unroll
   for (int j = 0; j < P; ++j) {
     const int pix = (iy0 + j * YSTEP) * L + ix;
@@ -175,8 +184,11 @@ __global__ void __launch_bounds__(T) gridder_kernel(const SubgridJob job, const 
 #pragma unroll
     for (int p = 0; p < 4; ++p)
       x[p] = (j & 1) ? make_float2(are[p][j / 2].y, aim[p][j / 2].y) : make_float2(are[p][j / 2].x, aim[p][j / 2].x);
-    sandwich(x, __ldg(&ap[pix * 2]), __ldg(&ap[pix * 2 + 1]), __ldg(&aq[pix * 2]), __ldg(&aq[pix * 2 + 1]),
-             __ldg(&job.taper[pix]), z);
+    const float4 mp0 = __ldg(&ap[pix * 2]), mp1 = __ldg(&ap[pix * 2 + 1]);
+    const float4 mq0 = __ldg(&aq[pix * 2]), mq1 = __ldg(&aq[pix * 2 + 1]);
+    float t = __ldg(&job.taper[pix]);
+    if (job.power_norm) t *= frobenius_inv(mp0, mp1, mq0, mq1);        // PAPER.md:257, R22
+    sandwich(x, mp0, mp1, mq0, mq1, t, z);
 #pragma unroll
     for (int p = 0; p < 4; ++p) o[p * L * L + pix] = z[p];
   }
@@ -189,6 +201,7 @@ cudaError_t launch(const SubgridJob& job, const float4* vis, float2* out, cudaSt
   if (blocks == 0) return cudaSuccess;
   gridder_kernel<L, T, P><<<static_cast<unsigned>(blocks), T, 0, stream>>>(job, vis, out);
   count_launch();
+  note_kernel(IDG_K_GRIDDER, IDG_KMASK_SIMT);
   return cudaGetLastError();
 }
 
@@ -197,9 +210,11 @@ cudaError_t launch(const SubgridJob& job, const float4* vis, float2* out, cudaSt
 cudaError_t launch_gridder(const SubgridJob& job, const float4* vis, float2* out, cudaStream_t stream) {
   switch (job.subgrid_size) {
     case 32:  return launch<32, 128, 8>(job, vis, out, stream);
+    case 48:  return launch<48, 192, 6>(job, vis, out, stream);
     case 64:  return launch<64, 256, 8>(job, vis, out, stream);
     case 96:  return launch<96, 384, 8>(job, vis, out, stream);
     case 128: return launch<128, 256, 8>(job, vis, out, stream);
+    case 160: return launch<160, 320, 8>(job, vis, out, stream);
     default:  return cudaErrorInvalidValue;
   }
 }

@@ -82,10 +82,11 @@ constexpr int kVisBytes = 64;            // B operand bytes per visibility: 2 k-
 constexpr int kVisBytes = 128;           // 2 k-rows x 16 columns x 4 bytes
 #endif
 
-struct RowDataTc {
+struct alignas(16) RowDataTc {     // 32 bytes: two 128-bit shared-memory loads
   int32_t alpha_fix, beta_fix;   // (u-u0) S/L and (v-v0) S/L at kappa_ref, cycles/pixel * 2^32 (wrapping)
   float gamma;                   // 2 pi (w kappa_ref - w0)
   float us, vs, ws;              // 2 pi u_m S/L, 2 pi v_m S/L, 2 pi w_m   [rad per unit kappa]
+  float dmax;                    // bound of |pa * dkappa| over the subgrid's pixels: the phase step per channel [rad]
 };
 
 // tf32-exact head of x (the low 13 mantissa bits cleared); x - head is exact in fp32
@@ -95,8 +96,9 @@ struct RowDataTc {
 }
 
 // NG = compute groups (tiles in flight) per CTA, KC = visibilities per chunk, DG = chunks per accumulator
-// group, NA = depth of a group's A ring in TMEM
-template <int L, int NG, int KC, int DG, int NA>
+// group, NA = depth of a group's A ring in TMEM, ROT = phasors by rotation along the channel axis (uniformly
+// spaced channels, job.dkappa != 0) instead of one __sincosf per (visibility, pixel) pair
+template <int L, int NG, int KC, int DG, int NA, bool ROT>
 __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ? 2 : 1))
     gridder_tc_kernel(const SubgridJob job, const float4* __restrict__ vis, float2* __restrict__ out,
                       const int cap_chunks) {
@@ -105,8 +107,7 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
   constexpr int ROUNDS = TILES / NG;
   constexpr int NTHREADS = NG * kTileM + NG * 32;
 #ifdef IDG_TC_FP16
-  static_assert(KC == 8, "fp16 operands: 8-channel chunks");
-  constexpr int A_COLS = 2 * KC;                       // per slot: 8 words of (cos, sin) heads, 8 of remainders
+  constexpr int A_COLS = 2 * KC;                       // per slot and 8 visibilities: 8 words of (cos, sin) heads, 8 of remainders
 #else
   constexpr int A_COLS = 4 * KC;                       // per slot: heads [0, 2KC), remainders [2KC, 4KC)
 #endif
@@ -136,10 +137,11 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
   __shared__ uint32_t s_vmax;                          // fp16 operands: bits of the segment's largest |component|
 
   const int tid = threadIdx.x, warp = tid / 32;
-  const int64_t sg = blockIdx.x;
+  const int64_t sg = job_slot(job, blockIdx.x);
   const int32_t* m = job.meta + (job.first + sg) * kMetaStride;
   const int b = m[0], t0 = m[1], nt = m[2], c0 = m[3], nc = m[4], x0 = m[5], y0 = m[6], wl = m[7];
   const int sp = m[8], sq = m[9], it = m[10];
+  const bool conj = (m[12] & kMetaConj) != 0;          // rows used as (-u,-v,-w) with V^dagger (PAPER.md:178 fn 4, R21)
   const int64_t row0 = static_cast<int64_t>(b) * job.n_times + t0;
 
   const uint32_t bar0 = tc::smem_u32(&bars[0]);
@@ -175,7 +177,8 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
       const double v0 = (y0 + L / 2 - job.grid_size / 2) / S;
       const double w0 = job.w_step > 0.0 ? (wl + 0.5) * job.w_step : 0.0;
       const double* uvw = job.uvw + (row0 + tid) * 3;
-      const double um = uvw[0], vm = uvw[1], wm = uvw[2];
+      const double sgn = conj ? -1.0 : 1.0;
+      const double um = sgn * uvw[0], vm = sgn * uvw[1], wm = sgn * uvw[2];
       const double two_pi = 6.283185307179586476925286766559;
       const double sl = S / L;
       const double alpha = (um * kref - u0) * sl, beta = (vm * kref - v0) * sl;
@@ -186,6 +189,9 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
       rd.us = static_cast<float>(two_pi * um * sl);
       rd.vs = static_cast<float>(two_pi * vm * sl);
       rd.ws = static_cast<float>(two_pi * wm);
+      // the corner pixel (0, 0) has the largest |l|, |m| and |n'|
+      rd.dmax = static_cast<float>(fabs(job.dkappa) * two_pi *
+                                   ((fabs(um) + fabs(vm)) * sl * (L / 2) + fabs(wm) * fabs(static_cast<double>(job.nprime[0]))));
       srow[tid] = rd;
     }
   }
@@ -217,6 +223,7 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
   const float4* __restrict__ aq = job.aterms + (static_cast<int64_t>(sq) * job.n_intervals + it) * (L * L * 2);
   float2* o = out + sg * 4 * L * L;
   const uint32_t sdk_addr = tc::opaque(tc::smem_u32(&sdk[0]));
+  [[maybe_unused]] const float dkf = static_cast<float>(job.dkappa);   // channel spacing in kappa (ROT)
 
   for (int seg = 0; seg < nseg; ++seg) {
     const int r_begin = seg * rows_per_seg, r_end = min(nt, r_begin + rows_per_seg);
@@ -228,6 +235,12 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
     if (seg > 0) __syncthreads();                      // every MMA of the previous segment was drained
     // One warp per 8 visibilities x 4 polarisations, so the row / channel split is once per warp.
     constexpr int UPC = KC / 8;
+    // polarisation p of visibility (row r, channel c) as the sum uses it: V, or V^dagger = conj of (XX, YX, XY, YY)
+    auto load_vis = [&](int r, int c, int p) -> float2 {
+      const int ps = conj ? ((p == 1 || p == 2) ? 3 - p : p) : p;
+      const float2 v = __ldg(reinterpret_cast<const float2*>(vis) + ((row0 + r) * job.n_chan + c0 + c) * 4 + ps);
+      return conj ? make_float2(v.x, -v.y) : v;
+    };
     // the chunk count is padded to whole ring revolutions with zero chunks (B = 0 contributes nothing), so
     // neither the compute threads nor the service warp ever test whether a slot is in use
     const int nchunks_pad = (nchunks + NA - 1) / NA * NA;
@@ -242,7 +255,7 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
         const int rr = ci / cpr;
         const int r = r_begin + rr, cc = (ci - rr * cpr) * KC;
         if (cc + j < nc) {
-          float2 v = __ldg(reinterpret_cast<const float2*>(vis) + ((row0 + r) * job.n_chan + c0 + cc + j) * 4 + p);
+          float2 v = load_vis(r, cc + j, p);
           if (job.weights != nullptr) {
             const float wgt = __ldg(&job.weights[(row0 + r) * job.n_chan + c0 + cc + j]);
             v = make_float2(v.x * wgt, v.y * wgt);
@@ -264,7 +277,7 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
       const int r = r_begin + rr, cc = (ci - rr * cpr) * KC;
       float2 v = make_float2(0.f, 0.f);
       if (ci < nchunks && cc + j < nc) {
-        v = __ldg(reinterpret_cast<const float2*>(vis) + ((row0 + r) * job.n_chan + c0 + cc + j) * 4 + p);
+        v = load_vis(r, cc + j, p);
         if (job.weights != nullptr) {
           const float wgt = __ldg(&job.weights[(row0 + r) * job.n_chan + c0 + cc + j]);
           v = make_float2(v.x * wgt, v.y * wgt);
@@ -291,7 +304,7 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
       const int r = r_begin + rr, cc = (ci - rr * cpr) * KC;
       float2 v = make_float2(0.f, 0.f);
       if (ci < nchunks && cc + j < nc) {
-        v = __ldg(reinterpret_cast<const float2*>(vis) + ((row0 + r) * job.n_chan + c0 + cc + j) * 4 + p);
+        v = load_vis(r, cc + j, p);
         if (job.weights != nullptr) {                  // weighting at load
           const float wgt = __ldg(&job.weights[(row0 + r) * job.n_chan + c0 + cc + j]);
           v = make_float2(v.x * wgt, v.y * wgt);
@@ -340,8 +353,11 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
             if (tc::elect_one()) {
 #ifdef IDG_TC_FP16
 #pragma unroll
-              for (int part = 0; part < 2; ++part)      // heads, remainders: one K = 16 MMA each
-                tc::mma_f16_ts(d0, gt + s * A_COLS + part * KC, bdesc0, IDESC, (rig > 0 || s > 0 || part > 0) ? 1u : 0u);
+              for (int half = 0; half < KC / 8; ++half)   // 8 visibilities = 16 k-rows of B, 512 bytes on
+#pragma unroll
+                for (int part = 0; part < 2; ++part)      // heads, remainders: one K = 16 MMA each
+                  tc::mma_f16_ts(d0, gt + s * A_COLS + half * 16 + part * 8, bdesc0 + half * (512 >> 4), IDESC,
+                                 (rig > 0 || s > 0 || half > 0 || part > 0) ? 1u : 0u);
 #else
 #pragma unroll
               for (int part = 0; part < 2; ++part)
@@ -391,8 +407,11 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
           }
         }
         if (last_seg) {
-          sandwich(x, __ldg(&ap[pix * 2]), __ldg(&ap[pix * 2 + 1]), __ldg(&aq[pix * 2]), __ldg(&aq[pix * 2 + 1]),
-                   __ldg(&job.taper[pix]), z);
+          const float4 mp0 = __ldg(&ap[pix * 2]), mp1 = __ldg(&ap[pix * 2 + 1]);
+          const float4 mq0 = __ldg(&aq[pix * 2]), mq1 = __ldg(&aq[pix * 2 + 1]);
+          float t = __ldg(&job.taper[pix]);
+          if (job.power_norm) t *= frobenius_inv(mp0, mp1, mq0, mq1);    // PAPER.md:257, R22
+          sandwich(x, mp0, mp1, mq0, mq1, t, z);
 #pragma unroll
           for (int p = 0; p < 4; ++p) o[p * L * L + pix] = z[p];
         } else {
@@ -414,11 +433,42 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
         for (int n = 0; n < 8; ++n) acc[n] = 0.f;
         // per-(row, pixel) slope and offset of the phase; amortised over the row's channels
         float pa, pb;
+        // ROT: the phase is linear in the channel, phi(c + 1) = phi(c) + delta with delta = pa * dkappa per (row,
+        // pixel), so e(c + 1) = e(c) rot, rot = exp(i delta) (the per-row precomputation, one step
+        // further).  Kept as kh = 1 - cos(delta) and sg = sin(delta), both to RELATIVE fp32 accuracy (a rotor error
+        // grows linearly along the chain): Taylor series at delta / 4 and two angle doublings for |delta| < 3,
+        // the accurate sincosf beyond (short rows of long baselines).
+        [[maybe_unused]] float2 nk2 = make_float2(0.f, 0.f);     // (-2 kh, -2 kh) = -4 sin^2(delta / 2)
+        [[maybe_unused]] float kh = 0.f, sg = 0.f;
         auto row_setup = [&](int r) {
           const RowDataTc rd = srow[r];
           pa = fmaf(rd.vs, static_cast<float>(iy), fmaf(rd.ws, np, rd.us * static_cast<float>(ix)));
           const int32_t bf = rd.alpha_fix * ix + rd.beta_fix * iy;                  // wraps: exact mod 1 cycle
           pb = fmaf(rd.gamma, np, static_cast<float>(bf) * 1.4629180792671596e-9f);   // 2 pi / 2^32
+          if constexpr (ROT) {
+            const float delta = pa * dkf;
+            if (rd.dmax < 3.0f) {                        // CTA-uniform
+              const float x = 0.25f * delta, t = x * x;
+              // sin x = x (1 - t/6 + t^2/120 - t^3/5040 + t^4/362880), 1 - cos x = t (1/2 - t/24 + t^2/720 - t^3/40320)
+              float s1 = fmaf(t, 2.7557319e-6f, -1.9841270e-4f);
+              s1 = fmaf(t, s1, 8.3333333e-3f);
+              s1 = fmaf(t, s1, -1.6666667e-1f);
+              s1 = fmaf(x * t, s1, x);
+              float k1 = fmaf(t, -2.4801587e-5f, 1.3888889e-3f);
+              k1 = fmaf(t, k1, -4.1666667e-2f);
+              k1 = fmaf(t, k1, 0.5f);
+              k1 *= t;
+              // doubling: sin 2x = 2 s (1 - k), 1 - cos 2x = 2 s^2
+              const float s2 = 2.f * s1 * (1.f - k1), k2 = 2.f * s1 * s1;
+              sg = 2.f * s2 * (1.f - k2);
+              kh = 2.f * s2 * s2;
+            } else {
+              float c;
+              sincosf(delta, &sg, &c);
+              kh = 1.f - c;
+            }
+            nk2 = make_float2(-2.f * kh, -2.f * kh);
+          }
         };
         int r = r_begin, cc = 0;
         row_setup(r);
@@ -432,7 +482,33 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
             // issued a whole hand-off / wait / store sequence ago
             if (s > 0) hand_off(gbar + 8 * (s - 1));
             else if (pending) hand_off(gbar + 8 * (NA - 1));
-            uint32_t hi[KC / 8][16], lo[KC / 8][16];
+            uint32_t hi[KC / 8][16];
+            [[maybe_unused]] uint32_t lo[KC / 8][16];
+#ifdef IDG_TC_FP16
+            if constexpr (ROT) {
+              // one __sincosf per 8 channels (which bounds the growth of rounding errors), then 7 rotations:
+              // d(c + 1) = d(c) - 4 sin^2(delta / 2) e(c), e(c + 1) = e(c) + d(c + 1), d(1) = e(0) (rot - 1),
+              // both components of e = (cos, sin) in one packed instruction each
+#pragma unroll
+              for (int half = 0; half < KC / 8; ++half) {
+                const float ph = fmaf(pa, tc::lds32(dk_addr + half * 32), pb);
+                float2 e;
+                __sincosf(ph, &e.y, &e.x);
+                float2 d = make_float2(fmaf(-kh, e.x, -sg * e.y), fmaf(-kh, e.y, sg * e.x));
+                const float2 m1 = make_float2(-1.f, -1.f);
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                  if (j == 1) e = __fadd2_rn(e, d);
+                  if (j > 1) { d = ffma2(e, nk2, d); e = __fadd2_rn(e, d); }
+                  const __half2 q = __floats2half2_rn(e.x, e.y);
+                  const float2 l = ffma2(__half22float2(q), m1, e);
+                  const __half2 rr = __floats2half2_rn(l.x, l.y);
+                  hi[half][j] = *reinterpret_cast<const uint32_t*>(&q);
+                  hi[half][8 + j] = *reinterpret_cast<const uint32_t*>(&rr);
+                }
+              }
+            } else
+#endif
             if (valid) {
 #pragma unroll
               for (int half = 0; half < KC / 8; ++half) {
@@ -479,16 +555,18 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
             if (valid) {
 #pragma unroll
               for (int half = 0; half < KC / 8; ++half) {
-                if constexpr (KC == 8) {
 #ifdef IDG_TC_FP16
-                  tc::tmem_st16(gtmem + s * A_COLS, hi[half]);               // 8 head words, 8 remainder words
+                // per 8 visibilities: 8 head words, 8 remainder words (16 columns)
+                if constexpr (KC == 8) tc::tmem_st16(gtmem + s * A_COLS, hi[half]);
+                else if (half == 0) tc::tmem_st32(gtmem + s * A_COLS, hi[0], hi[KC / 8 - 1]);
 #else
+                if constexpr (KC == 8) {
                   tc::tmem_st32(gtmem + s * A_COLS, hi[half], lo[half]);     // heads and remainders are adjacent
-#endif
                 } else {
                   tc::tmem_st16(gtmem + s * A_COLS + half * 16, hi[half]);
                   tc::tmem_st16(gtmem + s * A_COLS + 2 * KC + half * 16, lo[half]);
                 }
+#endif
               }
               dk_addr += KC * 4;
               cc += KC;
@@ -530,8 +608,8 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
   if (warp == NG * 4) tc::tmem_dealloc(tmem, TMEM_COLS);
 }
 
-template <int L, int NG, int KC, int DG, int NA>
-cudaError_t launch(const SubgridJob& job, const float4* vis, float2* out, cudaStream_t stream) {
+template <int L, int NG, int KC, int DG, int NA, bool ROT>
+cudaError_t launch_rot(const SubgridJob& job, const float4* vis, float2* out, cudaStream_t stream) {
   if (job.count == 0) return cudaSuccess;
 #ifdef IDG_TC_FP16
   constexpr int CHUNK_BYTES = KC * 64;
@@ -541,17 +619,23 @@ cudaError_t launch(const SubgridJob& job, const float4* vis, float2* out, cudaSt
   const int cpr_max = (job.n_chan + KC - 1) / KC;
   const int cap_chunks = std::min(job.max_nt * cpr_max, kMaxBBytes / CHUNK_BYTES);
   const size_t dyn = static_cast<size_t>(cap_chunks + NA - 1) * CHUNK_BYTES;   // + padding chunks
-  auto kernel = gridder_tc_kernel<L, NG, KC, DG, NA>;
-  static size_t configured = 0;                        // per instantiation
-  if (dyn > configured) {
-    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         kMaxBBytes + (NA - 1) * CHUNK_BYTES);
-    if (e != cudaSuccess) return e;
-    configured = kMaxBBytes;
-  }
+  auto kernel = gridder_tc_kernel<L, NG, KC, DG, NA, ROT>;
+  // per launch: the attribute belongs to the (function, device) pair and the call is cheap
+  cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn));
+  if (e != cudaSuccess) return e;
   kernel<<<static_cast<unsigned>(job.count), NG * kTileM + NG * 32, dyn, stream>>>(job, vis, out, cap_chunks);
   count_launch();
+  note_kernel(IDG_K_GRIDDER, IDG_KMASK_TC(NG));
   return cudaGetLastError();
+}
+
+// Rotation along the channel axis needs uniformly spaced channels (job.dkappa != 0, checked by the planner).
+template <int L, int NG, int KC, int DG, int NA>
+cudaError_t launch(const SubgridJob& job, const float4* vis, float2* out, cudaStream_t stream) {
+#if defined(IDG_TC_FP16) && !defined(IDG_TC_NOROT)
+  if (job.dkappa != 0.0) return launch_rot<L, NG, KC, DG, NA, true>(job, vis, out, stream);
+#endif
+  return launch_rot<L, NG, KC, DG, NA, false>(job, vis, out, stream);
 }
 
 // Groups per CTA.  Tensor memory holds four groups per SM whatever the split; with fewer groups per CTA
@@ -568,8 +652,10 @@ cudaError_t launch_l(const SubgridJob& job, const float4* vis, float2* out, cuda
   return launch<L, IDG_TC_NG, KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
 #else
   if (4 * (dyn + kStaticAndReserved) <= kSmemPerSm) return launch<L, 1, KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
-  if (2 * (dyn + kStaticAndReserved) <= kSmemPerSm) return launch<L, 2, KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
-  return launch<L, 4, KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
+  if (2 * (dyn + kStaticAndReserved) <= kSmemPerSm || ((L * L) / kTileM) % 4 != 0)     // L = 48: 18 tiles
+    return launch<L, 2, KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
+  if constexpr (((L * L) / kTileM) % 4 == 0) return launch<L, 4, KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
+  return cudaErrorInvalidValue;
 #endif
 }
 
@@ -583,9 +669,11 @@ cudaError_t launch_gridder_tc(const SubgridJob& job, const float4* vis, float2* 
     return launch_gridder(job, vis, out, stream);
   switch (job.subgrid_size) {
     case 32:  return launch_l<32>(job, vis, out, stream);
+    case 48:  return launch_l<48>(job, vis, out, stream);
     case 64:  return launch_l<64>(job, vis, out, stream);
     case 96:  return launch_l<96>(job, vis, out, stream);
     case 128: return launch_l<128>(job, vis, out, stream);
+    case 160: return launch_l<160>(job, vis, out, stream);
     default:  return cudaErrorInvalidValue;
   }
 }

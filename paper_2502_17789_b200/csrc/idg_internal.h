@@ -12,9 +12,11 @@
 namespace idg {
 
 constexpr double kSpeedOfLight = 299792458.0;
-constexpr int kMetaStride = 12;   // int32 per subgrid on the device: b,t0,nt,c0,nc,x0,y0,wl,p,q,it,layer
+constexpr int kMetaStride = 16;   // int32 per subgrid on the device: b,t0,nt,c0,nc,x0,y0,wl,p,q,it,layer,flags,-,-,-
+constexpr int kMetaConj = 1;      // flags bit 0: rows are used conjugated, (u,v,w) -> -(u,v,w), V -> V^dagger (R21); p,q already swapped
 constexpr int kTile = 32;         // adder tile edge in master-grid pixels
 constexpr int kAdderSegment = 128;   // subgrids one adder block walks; longer tile lists are split
+constexpr int kDegridTensorMin = 48;   // visibilities from which a subgrid takes the tensor-core degridder under AUTO
 constexpr int kSegStride = 6;     // int32 per adder segment: tile index, begin, end, k, n_seg, partial slot
 
 // tile -> subgrid lists for the atomic-free adder (one CSR per batch of subgrids).
@@ -39,9 +41,26 @@ struct DeviceCsr {
   int32_t* counters = nullptr;     // [n_tiles] segments finished per tile, zero between launches
 };
 
+// Which subgrids of a range go to which direct-sum kernel (IDG_VARIANT_AUTO decides per subgrid,
+// PAPER.md:247 fn 7).  Indices are relative to the range's first subgrid; an empty `tensor` AND empty
+// `simt` list never occurs for a non-empty range.  When one list is empty the other launch needs no
+// indirection.
+struct KernelSplit {
+  std::vector<int32_t> tensor, simt;
+  int variant = 0;                 // the plan's IDG_VARIANT_* for this step (FP64 and forced variants: no lists)
+};
+
 struct Batch {
   int64_t first = 0, count = 0;
   TileCsr csr;
+  KernelSplit grid_split, degrid_split;
+};
+
+struct DeviceSplit {
+  int32_t* tensor = nullptr;       // device copies of KernelSplit's lists (nullptr when not mixed)
+  int32_t* simt = nullptr;
+  int32_t n_tensor = 0, n_simt = 0;
+  int variant = 0;
 };
 
 struct DeviceState {
@@ -50,6 +69,7 @@ struct DeviceState {
   int32_t* meta = nullptr;      // [n_subgrids, kMetaStride]
   float* nprime = nullptr;      // [L, L] n'(l, m) at the subgrid pixels
   std::vector<DeviceCsr> batch_csr;
+  std::vector<DeviceSplit> batch_grid_split, batch_degrid_split;
   double* adder_partials = nullptr;   // shared by the batches: sized for the largest
   int32_t* adder_counters = nullptr;
   void* closure_fft = nullptr;        // cuFFT plan of the master-grid transform, created on first use
@@ -65,6 +85,7 @@ struct idg_plan {
   double image_size = 0.0;                // S = Ng * cell
   std::vector<double> uvw;                // host copy [n_rows*3]
   std::vector<double> kappa;              // nu_c / c
+  double dkappa = 0.0;                    // channel spacing in kappa when uniform (to 1e-9 of the band), else 0
   std::vector<int32_t> baselines;         // [n_bl*2]
   std::vector<int32_t> sub;               // [n_subgrids*8]
   int64_t n_subgrids = 0, n_vis_planned = 0, n_vis_dropped = 0;
@@ -88,5 +109,7 @@ void set_error(const std::string& msg);
 int  plan_build(idg_plan* plan);
 void build_tile_csr(const idg_plan* plan, int64_t first, int64_t count, TileCsr* out);
 void fill_meta(const idg_plan* plan, std::vector<int32_t>* meta);
+bool subgrid_conjugated(const idg_plan* plan, const int32_t* sub8);
+void split_kernels(const idg_plan* plan, int64_t first, int64_t count, int direction, KernelSplit* out);
 
 }  // namespace idg

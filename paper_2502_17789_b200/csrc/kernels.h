@@ -18,13 +18,22 @@ struct SubgridJob {
   const float4* aterms;     // [n_st, n_int, L, L, 2] rows of the 2x2 Jones matrices
   const float* taper;       // [L, L]
   const float* weights;     // [n_rows, n_chan] imaging weights applied at load, or nullptr
-  int64_t first;            // first subgrid (global index)
-  int64_t count;
+  int64_t first;            // first subgrid (global index) of the range the launch belongs to
+  int64_t count;            // blocks' worth of subgrids in this launch
+  const int32_t* index;     // nullptr: block i handles subgrid first + i; else first + index[i] (kernel choice
+                            // per subgrid, PAPER.md:247 fn 7); the subgrid's slot in the stack is the same offset
   int32_t subgrid_size, grid_size, n_times, n_chan, n_intervals;
   int32_t max_nt;           // upper bound of nt over subgrids = min(n_times, aterm_period)
   double image_size;        // S
   double w_step;
+  double dkappa;            // kappa[c + 1] - kappa[c] when the channels are uniformly spaced, else 0
+  int32_t power_norm;       // imaging: divide the sandwich by || M_p M_q^H ||_F per pixel (R22)
 };
+
+// offset of a block's subgrid within the launch's range
+__device__ __forceinline__ int64_t job_slot(const SubgridJob& job, unsigned block) {
+  return job.index != nullptr ? static_cast<int64_t>(job.index[block]) : static_cast<int64_t>(block);
+}
 
 // steps a1-a3: stage visibilities, direct sum (Eq. 10), A-term sandwich and taper.
 // out [count, 4, L, L] complex64.
@@ -68,6 +77,23 @@ cudaError_t launch_grid_to_image(void* fft_plan, const float2* grid, const float
                                  int Ng, int n_layers, int wl_min, double w_step, double S, cudaStream_t stream);
 cudaError_t launch_image_to_grid(void* fft_plan, const float2* image, const float* corr, float2* grid, int Ng,
                                  int n_layers, int wl_min, double w_step, double S, cudaStream_t stream);
+
+// fp64 SIMT variants of the two direct sums with their A-term / taper step (direct_f64.cu).
+// OUT / IN = double2 keeps fp64 end to end (stage calls), float2 rounds to the complex64 stack / table.
+cudaError_t launch_gridder_f64(const SubgridJob& job, const float4* vis, float2* out32, double2* out64, cudaStream_t stream);
+cudaError_t launch_degridder_f64(const SubgridJob& job, const float2* in32, const double2* in64, float4* vis32,
+                                 double2* vis64, cudaStream_t stream);
+
+// weighted average of 1 / || M_p M_q^H ||_F over (baseline, interval) pairs (R22):
+// pairs [n_pairs, 3] int32 (p, q, it), weights [n_pairs] double, avg [L*L] double = sum w f / sum w
+cudaError_t launch_power_norm_average(const float4* aterms, int L, int n_intervals, const int32_t* pairs,
+                                      const double* weights, int64_t n_pairs, double wsum, double* scratch,
+                                      double* avg, cudaStream_t stream);
+
+constexpr int kPowerNormSlices = 64;   // slices of the (p, q, it) list, each one partial sum per pixel
+
+// records which direct-sum kernel ran (idg_kernel_config_mask)
+void note_kernel(int kind, int bit);
 
 // Empirical FFMA / FFMA2 / MUFU rates per SM clock (peaks.cu); synchronous.
 cudaError_t measure_alu_peaks(double* out5);

@@ -38,16 +38,30 @@ int plan_build(idg_plan* plan) {
   const double comfort_span = par.comfort * span_max;
   const bool layered = par.w_step > 0.0;
 
+  // uniformly spaced channels let the tensor-core gridder rotate its phasors along the channel axis
+  plan->dkappa = 0.0;
+  if (nC >= 2) {
+    const double dk = (plan->kappa[nC - 1] - plan->kappa[0]) / (nC - 1);
+    bool uniform = dk > 0.0;
+    for (int32_t c = 0; c < nC && uniform; ++c)
+      uniform = std::fabs(plan->kappa[c] - (plan->kappa[0] + c * dk)) <= 1e-9 * dk * nC;
+    if (uniform) plan->dkappa = dk;
+  }
+
   std::vector<Emitted> out;
   std::vector<double> X(static_cast<size_t>(nT) * nC), Y(X.size());
   std::vector<int64_t> WL(X.size());
+  std::vector<char> FLIP(static_cast<size_t>(nT), 0);
   std::vector<WorkItem> work;
   int64_t dropped = 0;
 
   for (int32_t b = 0; b < par.n_baselines; ++b) {
     const double* rows = plan->uvw.data() + static_cast<size_t>(b) * nT * 3;
     for (int32_t t = 0; t < nT; ++t) {
-      const double um = rows[t * 3 + 0], vm = rows[t * 3 + 1], wm = rows[t * 3 + 2];
+      double um = rows[t * 3 + 0], vm = rows[t * 3 + 1], wm = rows[t * 3 + 2];
+      // PAPER.md:178 (fn 4): a row with w < 0 is used as the row (-u,-v,-w) of the swapped baseline (R21)
+      FLIP[t] = (par.positive_w != 0 && wm < 0.0) ? 1 : 0;
+      if (FLIP[t]) { um = -um; vm = -vm; wm = -wm; }
       for (int32_t c = 0; c < nC; ++c) {
         const double k = plan->kappa[c];
         const size_t i = static_cast<size_t>(t) * nC + c;
@@ -83,7 +97,7 @@ int plan_build(idg_plan* plan) {
         int32_t n = 1;
         while (t0 + n < tb) {
           const int32_t t = t0 + n;
-          if (WL[at(t, lo)] != wl0 || WL[at(t, c1)] != wl0) break;
+          if (WL[at(t, lo)] != wl0 || WL[at(t, c1)] != wl0 || FLIP[t] != FLIP[t0]) break;
           const double nxmin = std::min(xmin, std::min(X[at(t, lo)], X[at(t, c1)]));
           const double nxmax = std::max(xmax, std::max(X[at(t, lo)], X[at(t, c1)]));
           const double nymin = std::min(ymin, std::min(Y[at(t, lo)], Y[at(t, c1)]));
@@ -144,6 +158,8 @@ int plan_build(idg_plan* plan) {
     bt.first = first;
     bt.count = std::min(plan->batch_capacity, plan->n_subgrids - first);
     build_tile_csr(plan, bt.first, bt.count, &bt.csr);
+    split_kernels(plan, bt.first, bt.count, IDG_GRID, &bt.grid_split);
+    split_kernels(plan, bt.first, bt.count, IDG_DEGRID, &bt.degrid_split);
     plan->batches.push_back(std::move(bt));
   }
   return IDG_OK;
@@ -206,18 +222,43 @@ void build_tile_csr(const idg_plan* plan, int64_t first, int64_t count, TileCsr*
   }
 }
 
-// Per-subgrid device metadata: the 8 plan fields plus stations (p, q), A-term interval and
-// grid layer index, so kernels need no second lookup.
+bool subgrid_conjugated(const idg_plan* plan, const int32_t* e) {
+  if (!plan->par.positive_w) return false;
+  return plan->uvw[(static_cast<size_t>(e[0]) * plan->par.n_times + e[1]) * 3 + 2] < 0.0;
+}
+
+// Kernel choice per subgrid (PAPER.md:247 fn 7, :239-241).  The tensor-core
+// gridder pads every table row to whole 8-channel chunks and the tensor-core degridder works on warps of 32
+// visibilities inside tiles of 128, so sparsely filled subgrids go to the SIMT kernels, which have no padding.
+void split_kernels(const idg_plan* plan, int64_t first, int64_t count, int direction, KernelSplit* out) {
+  out->tensor.clear(); out->simt.clear();
+  out->variant = direction == IDG_GRID ? plan->par.gridder_variant : plan->par.degridder_variant;
+  if (out->variant != IDG_VARIANT_AUTO) return;
+  for (int64_t i = 0; i < count; ++i) {
+    const int32_t* e = &plan->sub[static_cast<size_t>(first + i) * 8];
+    const int32_t nt = e[2], nc = e[4];
+    bool tensor;
+    if (direction == IDG_GRID) tensor = 10 * nc >= 8 * ((nc + 7) / 8 * 8);          // chunk fill >= 80 %
+    else                       tensor = static_cast<int64_t>(nt) * nc >= kDegridTensorMin;
+    (tensor ? out->tensor : out->simt).push_back(static_cast<int32_t>(i));
+  }
+}
+
+// Per-subgrid device metadata: the 8 plan fields plus stations (p, q), A-term interval,
+// grid layer index and flags, so kernels need no second lookup.
 void fill_meta(const idg_plan* plan, std::vector<int32_t>* meta) {
   meta->resize(static_cast<size_t>(plan->n_subgrids) * kMetaStride);
   for (int64_t s = 0; s < plan->n_subgrids; ++s) {
     const int32_t* e = &plan->sub[static_cast<size_t>(s) * 8];
     int32_t* m = &(*meta)[static_cast<size_t>(s) * kMetaStride];
     for (int i = 0; i < 8; ++i) m[i] = e[i];
-    m[8] = plan->baselines[static_cast<size_t>(e[0]) * 2 + 0];
-    m[9] = plan->baselines[static_cast<size_t>(e[0]) * 2 + 1];
+    const bool conj = subgrid_conjugated(plan, e);     // conjugated rows belong to the swapped baseline (R21)
+    m[8] = plan->baselines[static_cast<size_t>(e[0]) * 2 + (conj ? 1 : 0)];
+    m[9] = plan->baselines[static_cast<size_t>(e[0]) * 2 + (conj ? 0 : 1)];
     m[10] = e[1] / plan->par.aterm_period;
     m[11] = e[7] - plan->wl_min;
+    m[12] = conj ? kMetaConj : 0;
+    m[13] = m[14] = m[15] = 0;
   }
 }
 

@@ -17,6 +17,7 @@ from .generate import (  # noqa: F401
     baselines,
     channel_freqs,
     hash_visibilities,
+    hash_visibilities_torch,
     kaiser_bessel_1d,
     make_observation,
     point_sources,

@@ -309,3 +309,35 @@ def source_visibilities_torch(uvw_rows: np.ndarray, freqs: np.ndarray, src: dict
             ph = torch.complex(torch.cos(ang), torch.sin(ang)) * spec[c][None, :]
             out[r0:r0 + chunk_rows, c, :] = (ph @ Bf).to(torch.complex64)
     return out
+
+
+def hash_visibilities_torch(n_rows: int, n_chan: int, seed: int, device, chunk_rows: int = 1 << 16):
+    """`hash_visibilities` for all rows 0..n_rows-1, evaluated with torch int64 arithmetic on `device` in row
+    chunks (two's-complement wrap-around = the uint64 recipe; shifts made logical by masking).  Bit-identical to
+    the numpy generator (tests/test_synth.py checks sampled rows).  Returns complex64 [n_rows, n_chan, 4]."""
+    import torch
+
+    def i64(x):                       # uint64 constant -> the int64 with the same bits
+        x = int(x) & 0xFFFFFFFFFFFFFFFF
+        return x - (1 << 64) if x >= (1 << 63) else x
+
+    def lsr(z, k):
+        return (z >> k) & ((1 << (64 - k)) - 1)
+
+    A, B, C = i64(_SM_A), i64(_SM_B), i64(_SM_C)
+    # (seed * A + A) mod 2^64 as a Python integer: torch cannot multiply by it without overflow warnings
+    off = i64((int(seed) * int(_SM_A) + int(_SM_A)) & 0xFFFFFFFFFFFFFFFF)
+    out = torch.empty((n_rows, n_chan, 4), dtype=torch.complex64, device=device)
+    ch = torch.arange(n_chan, dtype=torch.int64, device=device)
+    k = torch.arange(8, dtype=torch.int64, device=device)
+    for r0 in range(0, n_rows, chunk_rows):
+        rows = torch.arange(r0, min(n_rows, r0 + chunk_rows), dtype=torch.int64, device=device)
+        ctr = (rows[:, None, None] * n_chan + ch[None, :, None]) * 8 + k[None, None, :]
+        z = ctr + off
+        z = (z ^ lsr(z, 30)) * B
+        z = (z ^ lsr(z, 27)) * C
+        z = z ^ lsr(z, 31)
+        u24 = lsr(z, 40).to(torch.float32) * (2.0 ** -24)
+        f = (2.0 * u24 - 1.0).to(torch.float32).contiguous()
+        out[r0:r0 + rows.numel()] = torch.view_as_complex(f.view(rows.numel(), n_chan, 4, 2))
+    return out

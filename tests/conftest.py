@@ -34,13 +34,3 @@ def idg():
     import paper_2502_17789_b200 as pkg
     pkg.load_library()
     return pkg
-
-
-@pytest.fixture(autouse=True)
-def _default_kernel_variants(request):
-    """Tests that pick a kernel variant do not leak the choice into the next test."""
-    yield
-    if "idg" in request.fixturenames:
-        pkg = request.getfixturevalue("idg")
-        for kind in ("gridder", "degridder"):
-            pkg.set_kernel_variant(kind, pkg.VARIANT_AUTO)

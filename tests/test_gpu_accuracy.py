@@ -9,14 +9,20 @@ and the recovered flux at the source pixels, after the caller's 1 / (T_full n_vi
 truth.  The Kaiser-Bessel taper of the synthetic inputs (R15: beta = pi P / 2) sets the fp64 curve; the
 fp32 curve follows it down to the single-precision floor.
 
-    python tests/accuracy_sweep.py > profiles/accuracy_sweep_r01.md      (on the GPU box)
+As a test (`-m gpu`) it runs three of the cases and asserts the shape of the curve; run as a module it writes the
+whole table:
 
+    python -m tests.test_gpu_accuracy > profiles/accuracy_sweep_r02.md      (on the GPU box)
+
+It also holds the accuracy check that needs the fp64 CUDA kernels: the fp32 gridders against
+the fp64 gridder on ALL 56 896 subgrids of config 2, a size the numpy oracle cannot reach.
 Test infrastructure: it imports the oracle, so it lives under tests/.
 """
 import os
 import sys
 
 import numpy as np
+import pytest
 import torch
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
@@ -77,30 +83,66 @@ def one_case(idg, L, P, n_src=6, seed=17):
         e64 = max(e64, abs(est.real - truth[s]) / flux.max())
 
     dev = "cuda:0"
-    plan = idg.plan_from_config(cfg, obs.uvw, obs.freqs, obs.baselines)
-    cnt = plan.counts()
     to = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)  # noqa: E731
-    d_grid = torch.zeros((cnt.n_wlayers, 4, Ng, Ng), dtype=torch.complex64, device=dev)
-    ws = torch.empty(max(plan.workspace_bytes(), plan.closure_workspace_bytes()), dtype=torch.uint8, device=dev)
     e32 = {}
     for name, variant in (("simt", idg.VARIANT_SIMT), ("tensor", idg.VARIANT_TENSOR)):
-        idg.set_kernel_variant("gridder", variant)
-        d_grid.zero_()
+        plan = idg.plan_from_config(cfg, obs.uvw, obs.freqs, obs.baselines, gridder_variant=variant)
+        cnt = plan.counts()
+        d_grid = torch.zeros((cnt.n_wlayers, 4, Ng, Ng), dtype=torch.complex64, device=dev)
+        ws = torch.empty(max(plan.workspace_bytes(), plan.closure_workspace_bytes()), dtype=torch.uint8, device=dev)
         idg.grid(plan, to(vis.astype(np.complex64)), to(eye), to(taper), d_grid, ws)
         d_img = torch.zeros((4, Ng, Ng), dtype=torch.complex64, device=dev)
         idg.grid_to_image(plan, d_grid, d_img, ws, corr=to((1.0 / (np.outer(t1, t1) * cfg.n_vis)).astype(np.float32)))
         img = d_img.cpu().numpy()
         e32[name] = max(abs(img[0, jy[s], jx[s]].real - truth[s]) / flux.max() for s in range(n_src))
-    idg.set_kernel_variant("gridder", idg.VARIANT_AUTO)
     return len(sub), e64, e32["simt"], e32["tensor"]
+
+
+@pytest.mark.gpu
+def test_error_falls_with_padding_down_to_the_fp32_floor(idg):
+    """Shape of PAPER.md Fig. 3 (:299): the method's own (fp64) error falls by orders of magnitude with the padding;
+    the fp32 path follows it down to a floor near the paper's own single-precision figure (6e-6, :313)."""
+    rows = {(L, P): one_case(idg, L, P) for L, P in ((32, 4), (32, 12), (64, 20))}
+    e64 = [rows[k][1] for k in ((32, 4), (32, 12), (64, 20))]
+    assert e64[0] > 30 * e64[1] > 30 * 30 * e64[2], e64
+    for (L, P), (_, m64, simt, tensor) in rows.items():
+        assert simt <= max(3.0 * m64, 3e-6) and tensor <= max(3.0 * m64, 3e-6), (L, P, m64, simt, tensor)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("variant", ["simt", "tensor"])
+def test_fp32_gridders_against_fp64_on_every_subgrid_of_config2(idg, variant):
+    """accuracy at a size the numpy oracle cannot reach.  The fp64 CUDA gridder (itself within
+    1e-11 of the oracle, tests/test_gpu_parity.py::test_fp64_direct_sums) is the reference for the fp32 gridders
+    on ALL 56 896 subgrids of BASELINE.json configs[1]: the worst normalised error over every subgrid."""
+    dev = "cuda:0"
+    cfg = synth.get_config(2)
+    obs = synth.make_observation(cfg, vis="hash")
+    plan = idg.plan_from_config(cfg, obs.uvw, obs.freqs, obs.baselines,
+                                gridder_variant={"simt": idg.VARIANT_SIMT, "tensor": idg.VARIANT_TENSOR}[variant])
+    n, L = plan.counts().n_subgrids, cfg.subgrid_size
+    to = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)  # noqa: E731
+    d_vis, d_at, d_tp = to(obs.vis), to(obs.aterms), to(obs.taper)
+    worst, mean, chunk = 0.0, 0.0, 8192
+    for first in range(0, n, chunk):
+        count = min(chunk, n - first)
+        o64 = torch.empty((count, 4, L, L), dtype=torch.complex128, device=dev)
+        o32 = torch.empty((count, 4, L, L), dtype=torch.complex64, device=dev)
+        idg.grid_subgrids_f64(plan, first, count, d_vis, d_at, d_tp, o64)
+        idg.grid_subgrids(plan, first, count, d_vis, d_at, d_tp, o32, stage=idg.STAGE_GRIDDER)
+        err = (o32.to(torch.complex128) - o64).abs().reshape(count, -1).amax(dim=1) / o64.abs().reshape(count, -1).amax(dim=1)
+        worst = max(worst, float(err.max()))
+        mean += float(err.sum())
+    print(f"config 2, all {n} subgrids, {variant} gridder vs fp64 gridder: worst {worst:.2e}, mean {mean / n:.2e}")
+    assert worst <= 1e-5
 
 
 def main():
     from paper_2502_17789_b200 import build
     build.build()
     import paper_2502_17789_b200 as idg
-    print("# Accuracy against padding and subgrid size (tests/accuracy_sweep.py)\n")
-    print("Command (GPU box): `python tests/accuracy_sweep.py > profiles/accuracy_sweep_r01.md`.  10 stations, "
+    print("# Accuracy against padding and subgrid size (tests/test_gpu_accuracy.py)\n")
+    print("Command (GPU box): `python -m tests.test_gpu_accuracy > profiles/accuracy_sweep_r02.md`.  10 stations, "
           "16 x 2 s, 8 channels, grid 1024 x 1024 at 120 arcsec, 6 point sources of 1-10 Jy at image pixels, "
           "Kaiser-Bessel taper beta = pi P / 2.  Error = max over the sources of |recovered - direct sum| / "
           "brightest flux, the direct sum being the imaging equation evaluated on the same visibilities in "

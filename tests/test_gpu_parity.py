@@ -2,6 +2,8 @@
 the same seeded inputs.  Tolerance (BASELINE.json north_star): normalised max
 error max|gpu - oracle| / max|oracle| <= 1e-5 per subgrid (after the A-term/taper epilogue and
 after the FFT) and per subgrid's degridded visibilities; plan, adder and splitter bit-exact."""
+import dataclasses
+
 import numpy as np
 import pytest
 import torch
@@ -24,12 +26,17 @@ def dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).to(DEV)
 
 
+VAR = {"auto": 0, "simt": 1, "tensor": 2, "fp64": 3}
+
+
 def setup(idg, cfg, vis="hash", aterms="config", seed=0, **plan_kw):
     obs = synth.make_observation(cfg, vis=vis, with_aterms=(aterms == "config"))
     if aterms == "random":
         rng = np.random.default_rng(seed)
         obs.aterms = random_jones(rng, (cfg.n_stations, cfg.n_intervals, cfg.subgrid_size, cfg.subgrid_size))
     par = oracle_params(cfg)
+    if plan_kw.get("positive_w") or plan_kw.get("power_norm"):
+        par = dataclasses.replace(par, positive_w=bool(plan_kw.get("positive_w")), power_norm=bool(plan_kw.get("power_norm")))
     plan = idg.plan_from_config(cfg, obs.uvw, obs.freqs, obs.baselines, **plan_kw)
     sub = plan.export()
     return obs, par, plan, sub
@@ -53,13 +60,25 @@ CASES = [
     # more visibilities per subgrid than the tensor-core gridder keeps in shared memory: segmented path
     ("long-rows", lambda: synth.scaled(synth.get_config(1), n_stations=4, n_times=8, n_chan=220, chan_width_hz=1e3),
      "hash"),
+    # the launch configurations the full-size configs reach (the tensor-core gridder picks its compute groups
+    # per CTA, NG, by shared-memory fit; config 3 / 5 at full size: all 384 channels, 4 rows per A-term interval
+    # -> <96, 2>); occupancy 1 ... 1536 in ONE launch, so AUTO mixes both kernels
+    ("cfg3-384ch", lambda: synth.scaled(synth.get_config(3), n_stations=6, n_times=8), "hash"),
+    ("L64-ng2", lambda: synth.scaled(synth.get_config(2), n_stations=6, n_times=16, n_chan=96), "hash"),
+    ("L64-ng4", lambda: synth.scaled(synth.get_config(2), n_stations=6, n_times=8, n_chan=208, chan_width_hz=10e3),
+     "hash"),
+    ("L128-ng2", lambda: synth.scaled(synth.get_config(2), n_stations=6, n_times=8, n_chan=96, subgrid_size=128,
+                                      padding=24), "hash"),
+    # the two further subgrid sizes of PAPER.md Fig. 7 :363-369
+    ("L48", lambda: synth.scaled(synth.get_config(1), n_stations=7, n_times=16, n_chan=16, subgrid_size=48,
+                                 padding=10), "hash"),
+    ("L160", lambda: synth.scaled(synth.get_config(2), n_stations=5, n_times=8, n_chan=8, subgrid_size=160,
+                                  padding=24), "hash"),
 ]
 IDS = [c[0] for c in CASES]
-
-
-def request_variant(idg, variant, kind="gridder"):
-    """Select the kernel of one direct-sum step for one test; conftest restores the default afterwards."""
-    idg.set_kernel_variant(kind, {"simt": idg.VARIANT_SIMT, "tensor": idg.VARIANT_TENSOR}[variant])
+# compute groups per CTA the tensor-core gridder must take on these cases (asserted through idg_kernel_config_mask)
+EXPECT_NG = {"cfg2-10st": 1, "cfg3-384ch": 2, "L64-ng2": 2, "L64-ng4": 4, "L128-ng2": 2, "wide-rows": 2, "long-rows": 4,
+             "L48": 1, "L160": 1}
 
 
 def sample_subgrids(sub, n, seed=0):
@@ -73,52 +92,91 @@ def sample_subgrids(sub, n, seed=0):
     return sorted(pick)
 
 
-@pytest.mark.parametrize("variant", ["simt", "tensor"])
+def occupancy_picks(sub, n, seed=0):
+    """sample_subgrids plus, where the plan has them, subgrids of 1-7, 100-200 and the most visibilities."""
+    occ = sub[:, 2].astype(np.int64) * sub[:, 4]
+    picks = set(sample_subgrids(sub, n, seed))
+    for lo, hi in ((1, 7), (100, 200)):
+        hit = np.nonzero((occ >= lo) & (occ <= hi))[0]
+        picks.update(hit[:2].tolist())
+    return sorted(picks)
+
+
+@pytest.mark.parametrize("variant", ["simt", "tensor", "auto"])
 @pytest.mark.parametrize("name,make,vis", CASES, ids=IDS)
 def test_gridder_and_fft_per_subgrid(idg, name, make, vis, variant):
-    """Steps a1-a4 per subgrid, after the epilogue and after the FFT, for both gridder kernels."""
-    request_variant(idg, variant)
+    """Steps a1-a4 per subgrid, after the epilogue and after the FFT, for both gridder kernels and the
+    per-subgrid choice between them."""
     cfg = make()
-    obs, par, plan, sub = setup(idg, cfg, vis=vis)
+    obs, par, plan, sub = setup(idg, cfg, vis=vis, gridder_variant=VAR[variant])
     L = cfg.subgrid_size
     n = len(sub)
     d_vis, d_at, d_tp = dev(obs.vis), dev(obs.aterms), dev(obs.taper)
     out_img = torch.zeros((n, 4, L, L), dtype=torch.complex64, device=DEV)
     out_uv = torch.zeros_like(out_img)
+    idg.kernel_config_mask("gridder", reset=True)
     idg.grid_subgrids(plan, 0, n, d_vis, d_at, d_tp, out_img, stage=idg.STAGE_GRIDDER)
+    mask = idg.kernel_config_mask("gridder", reset=True)
     idg.grid_subgrids(plan, 0, n, d_vis, d_at, d_tp, out_uv, stage=idg.STAGE_FFT)
     torch.cuda.synchronize()
+    # which kernel ran: the tests must know what they exercised
+    nc = sub[:, 4]
+    fill_ok = 10 * nc >= 8 * ((nc + 7) // 8 * 8)
+    if variant == "simt" or name == "many-chan":
+        assert mask == idg.KMASK_SIMT, (name, variant, mask)
+    elif variant == "tensor":
+        assert mask & ~idg.KMASK_SIMT and not mask & idg.KMASK_SIMT, (name, variant, mask)
+        if name in EXPECT_NG:
+            assert mask == idg.kmask_tc(EXPECT_NG[name]), (name, mask)
+    else:
+        assert bool(mask & idg.KMASK_SIMT) == bool((~fill_ok).any()), (name, mask)
+        assert bool(mask & ~idg.KMASK_SIMT) == bool(fill_ok.any()), (name, mask)
+    if name == "cfg3-384ch":
+        occ = sub[:, 2].astype(np.int64) * nc
+        assert occ.min() <= 7 and occ.max() == 1536 and ((occ >= 100) & (occ <= 200)).any(), "occupancy spread"
+        if variant == "auto":
+            assert mask == idg.KMASK_SIMT | idg.kmask_tc(2), mask
     g_img = out_img.cpu().numpy()
     g_uv = out_uv.cpu().numpy()
     worst = (0.0, 0.0)
-    for s in sample_subgrids(sub, 12):
+    for s in occupancy_picks(sub, 12):
         Sp, Shat = orc.grid_subgrid(par, sub[s], obs.uvw, obs.freqs, obs.vis, obs.baselines, obs.aterms, obs.taper)
         e1 = nerr(np.moveaxis(g_img[s], 0, 2), Sp)
         e2 = nerr(np.moveaxis(g_uv[s], 0, 2), Shat)
         worst = (max(worst[0], e1), max(worst[1], e2))
         assert e1 <= TOL and e2 <= TOL, (name, s, sub[s].tolist(), e1, e2)
-    print(f"{name}: worst normalised error image {worst[0]:.2e} uv {worst[1]:.2e}")
+    print(f"{name}/{variant}: worst normalised error image {worst[0]:.2e} uv {worst[1]:.2e}")
 
 
-@pytest.mark.parametrize("variant", ["simt", "tensor"])
+@pytest.mark.parametrize("variant", ["simt", "tensor", "auto"])
 @pytest.mark.parametrize("name,make,vis", CASES, ids=IDS)
 def test_degridder_per_subgrid(idg, name, make, vis, variant):
-    """Steps a8-a9 per subgrid on random image-domain subgrids, for both degridder kernels."""
-    request_variant(idg, variant, kind="degridder")
+    """Steps a8-a9 per subgrid on random image-domain subgrids, for both degridder kernels and the per-subgrid
+    choice between them (occupancies from 1 to 1536 in one launch on cfg3-384ch)."""
     cfg = make()
-    obs, par, plan, sub = setup(idg, cfg, vis=None)
+    obs, par, plan, sub = setup(idg, cfg, vis=None, degridder_variant=VAR[variant])
     L = cfg.subgrid_size
     n = len(sub)
     rng = np.random.default_rng(7)
-    picks = sample_subgrids(sub, 10)
+    picks = occupancy_picks(sub, 10)
     S = np.zeros((n, 4, L, L), np.complex64)
     for s in picks:
         S[s] = (rng.standard_normal((4, L, L)) + 1j * rng.standard_normal((4, L, L))).astype(np.complex64)
     d_S, d_at, d_tp = dev(S), dev(obs.aterms), dev(obs.taper)
     d_vis = torch.full((cfg.n_rows, cfg.n_chan, 4), 7.0 + 0j, dtype=torch.complex64, device=DEV)
+    idg.kernel_config_mask("degridder", reset=True)
     idg.degrid_subgrids(plan, 0, n, d_S, d_at, d_tp, d_vis)
     torch.cuda.synchronize()
+    mask = idg.kernel_config_mask("degridder", reset=True)
+    occ = sub[:, 2].astype(np.int64) * sub[:, 4]
+    if variant == "simt":
+        assert mask == idg.KMASK_SIMT
+    elif variant == "tensor":
+        assert mask == idg.kmask_tc(2)
+    else:
+        assert bool(mask & idg.KMASK_SIMT) == bool((occ < 48).any()) and bool(mask & idg.kmask_tc(2)) == bool((occ >= 48).any())
     g = d_vis.cpu().numpy()
+    worst = 0.0
     for s in picks:
         b, t0, nt, c0, nc = (int(v) for v in sub[s][:5])
         Mp, Mq = orc.subgrid_jones(par, sub[s], obs.baselines, obs.aterms)
@@ -126,10 +184,12 @@ def test_degridder_per_subgrid(idg, name, make, vis, variant):
         ref = orc.degridder_subgrid(par, sub[s], obs.uvw, obs.freqs, Sp)
         r0 = b * cfg.n_times + t0
         e = nerr(g[r0:r0 + nt, c0:c0 + nc], ref)
+        worst = max(worst, e)
         assert e <= TOL, (name, s, sub[s].tolist(), e)
+    print(f"{name}/{variant}: worst normalised error of the predicted visibilities {worst:.2e}")
 
 
-@pytest.mark.parametrize("L", [32, 64, 96, 128])
+@pytest.mark.parametrize("L", [32, 48, 64, 96, 128, 160])
 def test_subgrid_fft_matches_oracle_and_inverts(idg, L):
     rng = np.random.default_rng(L)
     x = (rng.standard_normal((5, L, L)) + 1j * rng.standard_normal((5, L, L))).astype(np.complex64)
@@ -314,16 +374,28 @@ def test_empty_and_error_paths(idg):
     ws = torch.empty(plan.workspace_bytes(), dtype=torch.uint8, device=DEV)
     idg.grid(plan, d_vis, d_at, d_tp, d_grid, ws)
     assert idg.launch_count() == before + 3                          # gridder, fft, adder
+    # a plan without subgrids: every call is a no-op, the host-buffer ones included (round-1 advisor finding)
+    empty = idg.Plan(grid_size=cfg.grid_size, subgrid_size=L, padding=cfg.padding, cell_size=cfg.cell_size, w_step=0.0,
+                     n_stations=cfg.n_stations, n_times=cfg.n_times, n_chan=cfg.n_chan, aterm_period=cfg.aterm_period,
+                     uvw_m=np.zeros((0, 3)), freqs=obs.freqs, baselines=np.zeros((0, 2), np.int32))
+    e_vis = torch.zeros((0, cfg.n_chan, 4), dtype=torch.complex64)
+    h_grid = torch.full((1, 4, cfg.grid_size, cfg.grid_size), 2.0 + 1.0j, dtype=torch.complex64)
+    arena = torch.empty(max(empty.host_arena_bytes(), 256), dtype=torch.uint8, device=DEV)
+    before = idg.launch_count()
+    idg.grid_host(empty, e_vis, obs.aterms, obs.taper, h_grid, arena)
+    idg.degrid_host(empty, h_grid, obs.aterms, obs.taper, e_vis, arena)
+    idg.grid(empty, e_vis.to(DEV), d_at, d_tp, d_grid, ws)
+    assert idg.launch_count() == before and bool((h_grid == 2.0 + 1.0j).all())
+    assert empty.host_traffic_bytes(idg.IDG_GRID) == (0, 0)
 
 
 @pytest.mark.parametrize("variant", ["simt", "tensor"])
 def test_full_path_config2_shape(idg, variant):
     """The whole path on a config-2-shaped observation (64 x 64 subgrids, 32 channels, 256 visibilities per
     subgrid) small enough for the oracle to grid in full, with each pair of direct-sum kernels."""
-    request_variant(idg, variant, kind="gridder")
-    request_variant(idg, variant, kind="degridder")
     cfg = synth.scaled(synth.get_config(2), n_stations=8, n_times=16, grid_size=1024, cell_arcsec=120.0)
-    obs, par, plan, sub = setup(idg, cfg, vis="hash", max_batch_subgrids=11)
+    obs, par, plan, sub = setup(idg, cfg, vis="hash", max_batch_subgrids=11, gridder_variant=VAR[variant],
+                                degridder_variant=VAR[variant])
     cnt = plan.counts()
     Ng = cfg.grid_size
     d_vis, d_at, d_tp = dev(obs.vis), dev(obs.aterms), dev(obs.taper)
@@ -405,9 +477,8 @@ def test_full_size_config2_sampled(idg):
 def test_weighted_gridding(idg, variant):
     """SURVEY §8(f) NEXT-2, weights at load: idg_grid_weighted == the oracle on vis * weights,
     zero weights (flags) included."""
-    request_variant(idg, variant, kind="gridder")
     cfg = synth.scaled(synth.get_config(2), n_stations=7, n_times=16, grid_size=1024, cell_arcsec=120.0)
-    obs, par, plan, sub = setup(idg, cfg, vis="hash")
+    obs, par, plan, sub = setup(idg, cfg, vis="hash", gridder_variant=VAR[variant])
     cnt = plan.counts()
     rng = np.random.default_rng(21)
     wgt = rng.uniform(0.0, 2.0, (cfg.n_rows, cfg.n_chan)).astype(np.float32)
@@ -419,3 +490,185 @@ def test_weighted_gridding(idg, variant):
     ref = orc.grid(par, sub, obs.uvw, obs.freqs, obs.vis.astype(np.complex128) * wgt[:, :, None].astype(np.float64),
                    obs.baselines, obs.aterms, obs.taper)
     assert nerr(d_grid.cpu().numpy(), ref) <= TOL
+
+
+def test_tensor_gridder_dynamic_range(idg):
+    """The tensor-core gridder scales a segment's visibilities by ONE power of two into fp16 range (include/idg_b200.h,
+    IDG_VARIANT_TENSOR): with 1e6 of dynamic range inside one subgrid its error stays ~2^-22 of the segment's
+    largest component, i.e. inside the 1e-5 bar relative to max |subgrid value| (north_star's metric), while samples far
+    below the maximum keep that ABSOLUTE accuracy, not their own relative one.  This pins the documented behaviour."""
+    cfg = synth.scaled(synth.get_config(2), n_stations=6, n_times=16)
+    obs, par, plan, sub = setup(idg, cfg, vis="hash", gridder_variant=VAR["tensor"])
+    rng = np.random.default_rng(5)
+    amp = 10.0 ** rng.uniform(-6.0, 0.0, (cfg.n_rows, cfg.n_chan, 1))
+    amp[:: 7, 3] = 1.0                                     # every subgrid holds full-scale samples too
+    obs.vis = (obs.vis * amp).astype(np.complex64)
+    L, n = cfg.subgrid_size, len(sub)
+    out = torch.zeros((n, 4, L, L), dtype=torch.complex64, device=DEV)
+    idg.grid_subgrids(plan, 0, n, dev(obs.vis), dev(obs.aterms), dev(obs.taper), out, stage=idg.STAGE_GRIDDER)
+    g = out.cpu().numpy()
+    worst = 0.0
+    for s in sample_subgrids(sub, 8):
+        Sp, _ = orc.grid_subgrid(par, sub[s], obs.uvw, obs.freqs, obs.vis, obs.baselines, obs.aterms, obs.taper)
+        worst = max(worst, nerr(np.moveaxis(g[s], 0, 2), Sp))
+    print(f"dynamic range 1e6: worst normalised error {worst:.2e}")
+    assert worst <= TOL
+    # a subgrid of ONLY faint samples is scaled by its own maximum: relative accuracy is kept
+    faint = (obs.vis * 1e-6).astype(np.complex64)
+    idg.grid_subgrids(plan, 0, n, dev(faint), dev(obs.aterms), dev(obs.taper), out, stage=idg.STAGE_GRIDDER)
+    g = out.cpu().numpy()
+    for s in sample_subgrids(sub, 3):
+        Sp, _ = orc.grid_subgrid(par, sub[s], obs.uvw, obs.freqs, faint, obs.baselines, obs.aterms, obs.taper)
+        assert nerr(np.moveaxis(g[s], 0, 2), Sp) <= TOL
+
+
+@pytest.mark.parametrize("variant", ["simt", "tensor"])
+def test_degridder_edge_of_span(idg, variant):
+    """Visibilities at the very edge of the usable span of large subgrids (L = 128 and 160): the linear part of the
+    phase reaches ~200 rad there.  Both degridders reduce it modulo one cycle exactly in fixed point (round-1 advisor
+    finding), so the error must stay well inside the bar, not merely under it."""
+    for L, P in ((128, 24), (160, 24)):
+        cfg = synth.scaled(synth.get_config(2), n_stations=6, n_times=16, n_chan=16, subgrid_size=L, padding=P,
+                           disk_diameter_m=4000.0, chan_width_hz=1.5e6, dt_s=20.0, aterm_period=16)
+        obs, par, plan, sub = setup(idg, cfg, vis=None, degridder_variant=VAR[variant])
+        n = len(sub)
+        # the subgrids whose members lie farthest from the centre
+        kappa = obs.freqs / 299792458.0
+        S = cfg.image_size
+        far = []
+        for s in range(n):
+            b, t0, nt, c0, nc, x0, y0, _ = (int(v) for v in sub[s])
+            r0 = b * cfg.n_times + t0
+            X = obs.uvw[r0:r0 + nt, 0:1] * kappa[None, c0:c0 + nc] * S - (x0 + L // 2 - cfg.grid_size // 2)
+            Y = obs.uvw[r0:r0 + nt, 1:2] * kappa[None, c0:c0 + nc] * S - (y0 + L // 2 - cfg.grid_size // 2)
+            far.append(max(np.abs(X).max(), np.abs(Y).max()))
+        picks = np.argsort(far)[-6:].tolist()
+        assert max(far) > 0.3 * (L - P), "case must reach the outer part of the usable span (+-(L - P) / 2)"
+        rng = np.random.default_rng(L)
+        Sg = np.zeros((n, 4, L, L), np.complex64)
+        for s in picks:
+            Sg[s] = (rng.standard_normal((4, L, L)) + 1j * rng.standard_normal((4, L, L))).astype(np.complex64)
+        d_vis = torch.zeros((cfg.n_rows, cfg.n_chan, 4), dtype=torch.complex64, device=DEV)
+        idg.degrid_subgrids(plan, 0, n, dev(Sg), dev(obs.aterms), dev(obs.taper), d_vis)
+        g = d_vis.cpu().numpy()
+        worst = 0.0
+        for s in picks:
+            b, t0, nt, c0, nc = (int(v) for v in sub[s][:5])
+            Mp, Mq = orc.subgrid_jones(par, sub[s], obs.baselines, obs.aterms)
+            Sp = orc.aterm_taper(np.moveaxis(Sg[s].astype(np.complex128), 0, 2), Mp, Mq, obs.taper)
+            ref = orc.degridder_subgrid(par, sub[s], obs.uvw, obs.freqs, Sp)
+            r0 = b * cfg.n_times + t0
+            worst = max(worst, nerr(g[r0:r0 + nt, c0:c0 + nc], ref))
+        print(f"L = {L} {variant}: worst edge-of-span error {worst:.2e}")
+        assert worst <= 3e-6
+
+
+def layered_config():
+    return synth.scaled(synth.get_config(3), n_stations=7, n_times=8, n_chan=48, grid_size=1024, cell_arcsec=120.0,
+                        w_step=4.0, ha_mid_deg=30.0)
+
+
+@pytest.mark.parametrize("variant", ["simt", "tensor", "fp64"])
+def test_positive_w_conjugation(idg, variant):
+    """SURVEY 8(f) NEXT-2, PAPER.md:178 footnote 4 (R21): with positive_w the plan has only layers wl >= 0, rows with
+    w < 0 are gridded as (-u,-v,-w) of the swapped baseline with V^dagger, and prediction writes the dagger back.
+    Whole path against the oracle run with the same option (which P11 pins against Eq. 1)."""
+    cfg = layered_config()
+    obs, par, plan, sub = setup(idg, cfg, vis="hash", aterms="random", seed=3, positive_w=True, max_batch_subgrids=9,
+                                gridder_variant=VAR[variant], degridder_variant=VAR[variant])
+    cnt = plan.counts()
+    signed = idg.plan_from_config(cfg, obs.uvw, obs.freqs, obs.baselines).counts()
+    assert cnt.wl_min >= 0 and signed.wl_min < 0 and cnt.n_wlayers < signed.n_wlayers
+    n_conj = sum(orc.subgrid_conjugated(par, s, obs.uvw) for s in sub)
+    assert 0 < n_conj < len(sub), "case must mix conjugated and plain subgrids"
+    Ng = cfg.grid_size
+    d_vis, d_at, d_tp = dev(obs.vis), dev(obs.aterms), dev(obs.taper)
+    d_grid = torch.zeros((cnt.n_wlayers, 4, Ng, Ng), dtype=torch.complex64, device=DEV)
+    ws = torch.empty(plan.workspace_bytes(), dtype=torch.uint8, device=DEV)
+    idg.grid(plan, d_vis, d_at, d_tp, d_grid, ws)
+    ref = orc.grid(par, sub, obs.uvw, obs.freqs, obs.vis, obs.baselines, obs.aterms, obs.taper)
+    e_grid = nerr(d_grid.cpu().numpy(), ref)
+    G = ref.astype(np.complex64)
+    sentinel = 9.0 + 1.0j
+    d_out = torch.full((cfg.n_rows, cfg.n_chan, 4), sentinel, dtype=torch.complex64, device=DEV)
+    idg.degrid(plan, dev(G), d_at, d_tp, d_out, ws)
+    vref = orc.degrid(par, sub, obs.uvw, obs.freqs, G, obs.baselines, obs.aterms, obs.taper,
+                      out=np.full((cfg.n_rows, cfg.n_chan, 4), sentinel, np.complex128))
+    e_vis = nerr(d_out.cpu().numpy(), vref)
+    print(f"positive_w {variant}: grid {e_grid:.2e} vis {e_vis:.2e} ({n_conj} of {len(sub)} subgrids conjugated)")
+    assert e_grid <= TOL and e_vis <= TOL
+
+
+@pytest.mark.parametrize("variant", ["simt", "tensor", "fp64"])
+def test_power_normalisation(idg, variant):
+    """SURVEY 8(f) NEXT-2, PAPER.md:257 (R22): the imaging sandwich divided by || M_p M_q^H ||_F per pixel, and the
+    visibility-weighted average of that factor (idg_power_norm_average) the caller corrects the image with; both
+    against the oracle (pinned by P12).  Prediction is not normalised."""
+    cfg = synth.scaled(synth.get_config(2), n_stations=7, n_times=16, grid_size=1024, cell_arcsec=120.0)
+    obs, par, plan, sub = setup(idg, cfg, vis="hash", aterms="random", seed=8, power_norm=True,
+                                gridder_variant=VAR[variant])
+    cnt = plan.counts()
+    L, Ng, n = cfg.subgrid_size, cfg.grid_size, len(sub)
+    d_vis, d_at, d_tp = dev(obs.vis), dev(obs.aterms), dev(obs.taper)
+    out = torch.zeros((n, 4, L, L), dtype=torch.complex64, device=DEV)
+    idg.grid_subgrids(plan, 0, n, d_vis, d_at, d_tp, out, stage=idg.STAGE_GRIDDER)
+    g = out.cpu().numpy()
+    for s in sample_subgrids(sub, 6):
+        Sp, _ = orc.grid_subgrid(par, sub[s], obs.uvw, obs.freqs, obs.vis, obs.baselines, obs.aterms, obs.taper)
+        plain, _ = orc.grid_subgrid(dataclasses.replace(par, power_norm=False), sub[s], obs.uvw, obs.freqs, obs.vis,
+                                    obs.baselines, obs.aterms, obs.taper)
+        assert nerr(np.moveaxis(g[s], 0, 2), Sp) <= TOL
+        assert nerr(plain, Sp) > 0.05, "the normalisation must matter in this case"
+    d_grid = torch.zeros((cnt.n_wlayers, 4, Ng, Ng), dtype=torch.complex64, device=DEV)
+    ws = torch.empty(plan.workspace_bytes(), dtype=torch.uint8, device=DEV)
+    idg.grid(plan, d_vis, d_at, d_tp, d_grid, ws)
+    ref = orc.grid(par, sub, obs.uvw, obs.freqs, obs.vis, obs.baselines, obs.aterms, obs.taper)
+    assert nerr(d_grid.cpu().numpy(), ref) <= TOL
+    d_avg = torch.zeros((L, L), dtype=torch.float64, device=DEV)
+    idg.power_norm_average(plan, d_at, d_avg)
+    want = orc.power_norm_average(par, sub, obs.uvw, obs.baselines, obs.aterms)
+    assert np.abs(d_avg.cpu().numpy() - want).max() <= 1e-12 * np.abs(want).max()
+
+
+@pytest.mark.parametrize("name,make", [("cfg1", lambda: synth.get_config(1)),
+                                       ("cfg3-8st-layers", CASES[3][1]), ("L128", CASES[5][1])],
+                         ids=["cfg1", "cfg3-8st-layers", "L128"])
+def test_fp64_direct_sums(idg, name, make):
+    """the fp64 kernels against the oracle at 1e-11 on the two direct
+    sums with their A-term / taper step, complex128 out (idg_grid_subgrids_f64 / idg_degrid_subgrids_f64); and as
+    IDG_VARIANT_FP64 inside the complex64 path, where only the final rounding to complex64 is left (1e-7)."""
+    cfg = make()
+    obs, par, plan, sub = setup(idg, cfg, vis="hash", gridder_variant=VAR["fp64"], degridder_variant=VAR["fp64"])
+    L, n = cfg.subgrid_size, len(sub)
+    d_vis, d_at, d_tp = dev(obs.vis), dev(obs.aterms), dev(obs.taper)
+    out64 = torch.zeros((n, 4, L, L), dtype=torch.complex128, device=DEV)
+    out32 = torch.zeros((n, 4, L, L), dtype=torch.complex64, device=DEV)
+    idg.grid_subgrids_f64(plan, 0, n, d_vis, d_at, d_tp, out64)
+    idg.kernel_config_mask("gridder", reset=True)
+    idg.grid_subgrids(plan, 0, n, d_vis, d_at, d_tp, out32, stage=idg.STAGE_GRIDDER)
+    assert idg.kernel_config_mask("gridder", reset=True) == idg.KMASK_FP64
+    g64, g32 = out64.cpu().numpy(), out32.cpu().numpy()
+    picks = sample_subgrids(sub, 8)
+    rng = np.random.default_rng(2)
+    S = np.zeros((n, 4, L, L), np.complex128)
+    for s in picks:
+        Sp, _ = orc.grid_subgrid(par, sub[s], obs.uvw, obs.freqs, obs.vis, obs.baselines, obs.aterms, obs.taper)
+        assert nerr(np.moveaxis(g64[s], 0, 2), Sp) <= 1e-11, (name, s)
+        assert nerr(np.moveaxis(g32[s], 0, 2), Sp) <= 1e-7, (name, s)
+        S[s] = rng.standard_normal((4, L, L)) + 1j * rng.standard_normal((4, L, L))
+    v64 = torch.zeros((cfg.n_rows, cfg.n_chan, 4), dtype=torch.complex128, device=DEV)
+    v32 = torch.zeros((cfg.n_rows, cfg.n_chan, 4), dtype=torch.complex64, device=DEV)
+    idg.degrid_subgrids_f64(plan, 0, n, dev(S), d_at, d_tp, v64)
+    idg.degrid_subgrids(plan, 0, n, dev(S.astype(np.complex64)), d_at, d_tp, v32)
+    h64, h32 = v64.cpu().numpy(), v32.cpu().numpy()
+    for s in picks:
+        b, t0, nt, c0, nc = (int(v) for v in sub[s][:5])
+        Mp, Mq = orc.subgrid_jones(par, sub[s], obs.baselines, obs.aterms)
+        r0 = b * cfg.n_times + t0
+        ref = orc.degridder_subgrid(par, sub[s], obs.uvw, obs.freqs,
+                                    orc.aterm_taper(np.moveaxis(S[s], 0, 2), Mp, Mq, obs.taper))
+        assert nerr(h64[r0:r0 + nt, c0:c0 + nc], ref) <= 1e-11, (name, s)
+        ref32 = orc.degridder_subgrid(par, sub[s], obs.uvw, obs.freqs,
+                                      orc.aterm_taper(np.moveaxis(S[s].astype(np.complex64).astype(np.complex128), 0, 2),
+                                                      Mp, Mq, obs.taper))
+        assert nerr(h32[r0:r0 + nt, c0:c0 + nc], ref32) <= 1e-7, (name, s)

@@ -37,6 +37,8 @@ CASES = [
     ("ragged", lambda: synth.scaled(synth.get_config(1), n_stations=7, n_times=13, n_chan=5, aterm_period=3)),
     ("L128", lambda: synth.scaled(synth.get_config(2), n_stations=10, n_times=16, subgrid_size=128, padding=24)),
     ("drops", lambda: synth.scaled(synth.get_config(2), n_stations=12, n_times=8, grid_size=512, cell_arcsec=300.0)),
+    ("L48", lambda: synth.scaled(synth.get_config(1), subgrid_size=48, padding=10)),
+    ("L160", lambda: synth.scaled(synth.get_config(2), n_stations=8, n_times=8, subgrid_size=160, padding=24)),
 ]
 
 
@@ -62,6 +64,29 @@ def test_plan_bit_exact_vs_oracle(idg, name, make):
         assert W > 2, "case must exercise several w-layers"
 
 
+@pytest.mark.parametrize("name,make", [CASES[2], CASES[6]], ids=["cfg3-12st-layers", "drops"])
+def test_plan_positive_w_bit_exact_vs_oracle(idg, name, make):
+    """PAPER.md:178 (fn 4), R21: with positive_w the C++ planner and the oracle's still agree element for element,
+    only layers wl >= 0 remain, every visibility stays planned, and rows with w < 0 sit in subgrids of their own."""
+    import dataclasses
+    cfg = make()
+    obs = synth.make_observation(cfg, vis=None, with_aterms=False)
+    par = dataclasses.replace(oracle_params(cfg), positive_w=True)
+    sub_o, dropped_o = orc.plan(par, obs.uvw, obs.freqs, cfg.n_baselines)
+    plan = _plan(idg, cfg, obs, positive_w=True)
+    cnt = plan.counts()
+    assert np.array_equal(plan.export(), sub_o) and cnt.n_vis_dropped == dropped_o
+    assert cnt.wl_min >= 0
+    assert cnt.n_vis_planned + cnt.n_vis_dropped == cfg.n_vis
+    if name == "cfg3-12st-layers":
+        signed = _plan(idg, cfg, obs).counts()
+        assert signed.wl_min < 0 and cnt.n_wlayers < signed.n_wlayers, "conjugation must remove the negative layers"
+        w = obs.uvw[:, 2].reshape(cfg.n_baselines, cfg.n_times)
+        for b, t0, nt in sub_o[:, :3]:
+            sg = np.sign(w[b, t0:t0 + nt])
+            assert np.all(sg == sg[0]) or np.all(w[b, t0:t0 + nt] >= 0) or np.all(w[b, t0:t0 + nt] < 0)
+
+
 def test_workspace_follows_batch_capacity(idg):
     cfg = synth.get_config(1)
     obs = synth.make_observation(cfg, vis=None, with_aterms=False)
@@ -81,7 +106,9 @@ def test_argument_validation(idg):
     with pytest.raises(idg.IdgError, match="station index"):
         idg.plan_from_config(cfg, obs.uvw, obs.freqs, bad)
     with pytest.raises(idg.IdgError, match="code -2"):
-        idg.plan_from_config(synth.scaled(cfg, subgrid_size=48), obs.uvw, obs.freqs, obs.baselines)
+        idg.plan_from_config(synth.scaled(cfg, subgrid_size=40), obs.uvw, obs.freqs, obs.baselines)
+    with pytest.raises(idg.IdgError, match="kernel variant"):
+        idg.plan_from_config(cfg, obs.uvw, obs.freqs, obs.baselines, gridder_variant=7)
     with pytest.raises(idg.IdgError):
         idg.plan_from_config(synth.scaled(cfg, padding=40), obs.uvw, obs.freqs, obs.baselines)
 
@@ -96,6 +123,30 @@ def test_empty_plan(idg):
     cnt = plan.counts()
     assert (cnt.n_subgrids, cnt.n_wlayers, cnt.n_vis_planned, cnt.n_vis_dropped) == (0, 1, 0, 0)
     assert plan.export().shape == (0, 8)
+    # the host-buffer entry points must not index per-layer tables that were never built (round-1 advisor finding)
+    assert plan.host_traffic_bytes(idg.IDG_GRID) == (0, 0) and plan.host_traffic_bytes(idg.IDG_DEGRID) == (0, 0)
+
+
+def test_binding_checks_dtype_and_size(idg):
+    """The C ABI sees only pointers: the binding refuses arrays of the wrong dtype or element count."""
+    import torch
+    cfg = synth.get_config(1)
+    obs = synth.make_observation(cfg, vis=None, with_aterms=False)
+    plan = _plan(idg, cfg, obs)
+    L = cfg.subgrid_size
+    ok_vis = torch.zeros((cfg.n_rows, cfg.n_chan, 4), dtype=torch.complex64)
+    at = torch.zeros((cfg.n_stations, cfg.n_intervals, L, L, 2, 2), dtype=torch.complex64)
+    tp = torch.zeros((L, L), dtype=torch.float32)
+    grid = torch.zeros((1, 4, cfg.grid_size, cfg.grid_size), dtype=torch.complex64)
+    arena = type("FakeCuda", (), {"is_cuda": True})()       # only the checks before any device work are reached
+    with pytest.raises(ValueError, match="dtype float32"):
+        idg.grid_host(plan, ok_vis.real.contiguous().repeat(1, 1, 1), at, tp, grid, arena)
+    with pytest.raises(ValueError, match="elements, expected"):
+        idg.grid_host(plan, ok_vis[:-1], at, tp, grid, arena)
+    with pytest.raises(ValueError, match="aterms"):
+        idg.grid_host(plan, ok_vis, at[:, :1], tp, grid, arena)
+    with pytest.raises(ValueError, match="grid"):
+        idg.degrid_host(plan, grid[:, :2], at, tp, ok_vis, arena)
 
 
 def test_device_calls_fail_loudly_without_cuda_tensors(idg):

@@ -32,3 +32,28 @@ def random_jones(rng, shape, scale=0.3):
 def inner(a, b):
     """<a, b> = sum conj(a) b over every complex entry."""
     return np.vdot(np.asarray(a).ravel(), np.asarray(b).ravel())
+
+
+class OnDevice:
+    """numpy-style READ access to slices of a CUDA tensor.  The oracle only slices its big inputs (visibility
+    rows of a subgrid, the master-grid patch under a subgrid); at the full sizes of BASELINE.json configs 3-5
+    those arrays live on the device, and this hands the oracle the same numbers a slice at a time."""
+
+    def __init__(self, t):
+        self.t = t
+        self.shape = tuple(t.shape)
+
+    def __getitem__(self, idx):
+        return self.t[idx].cpu().numpy()
+
+
+def device_inner(a, b, chunk=1 << 24):
+    """<a, b> = sum conj(a) b over two equally shaped complex64 CUDA tensors, accumulated in fp64 in chunks."""
+    import torch
+    fa, fb = a.reshape(-1), b.reshape(-1)
+    acc = 0j
+    for i in range(0, fa.numel(), chunk):
+        x = fa[i:i + chunk].to(torch.complex128)
+        y = fb[i:i + chunk].to(torch.complex128)
+        acc += complex(torch.sum(torch.conj(x) * y).item())
+    return acc
