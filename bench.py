@@ -307,6 +307,7 @@ def kernel_rooflines(cfg, sub, n_wlayers, prof_ms, prof_n, steps, peaks, sm_mhz_
     return out, peak_tflops, flop, alg_bytes
 
 
+VARIANTS = {"auto": 0, "simt": 1, "tensor": 2, "fp64": 3}      # IDG_VARIANT_* of include/idg_b200.h
 OPERANDS = ("direct sums on tcgen05: gridder fp16 head + fp16 remainder of (cos, sin) and of the visibilities (one "
             "power-of-two scale per segment), degridder tf32 head + tf32 remainder; fp32 accumulation in tensor memory, "
             "drained into fp32 registers every 12 chunks; phase, sin/cos, A-term sandwich, FFT in fp32, adder sums in "
@@ -426,7 +427,8 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    plan = idg.plan_from_config(cfg, obs.uvw, obs.freqs, obs.baselines, max_batch_subgrids=args.max_batch)
+    variants = dict(gridder_variant=VARIANTS[args.gridder_variant], degridder_variant=VARIANTS[args.degridder_variant])
+    plan = idg.plan_from_config(cfg, obs.uvw, obs.freqs, obs.baselines, max_batch_subgrids=args.max_batch, **variants)
     sub = plan.export()
     cnt = plan.counts()
     Ng = cfg.grid_size
@@ -465,7 +467,8 @@ def run_ours(args):
         # also timed device-resident below, so the two legs can be compared on one configuration of the library.
         e2e_plan, same_plan_ms = plan, leg["ms_per_step"]
         if args.e2e_batch and not args.max_batch:
-            e2e_plan = idg.plan_from_config(cfg, obs.uvw, obs.freqs, obs.baselines, max_batch_subgrids=args.e2e_batch)
+            e2e_plan = idg.plan_from_config(cfg, obs.uvw, obs.freqs, obs.baselines, max_batch_subgrids=args.e2e_batch,
+                                            **variants)
             same = device_leg(idg, torch, cfg, e2e_plan, sub, cnt, d_vis, d_at, d_tp, args.steps, 1, stream, barrier, peaks)
             same_plan_ms = same["ms_per_step"]
         torch.cuda.empty_cache()
@@ -557,6 +560,9 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="wall-time target of the cpu_baseline leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--gridder-variant", default="auto", choices=["auto", "simt", "tensor", "fp64"],
+                    help="idg_params.gridder_variant (auto = per subgrid, the library default)")
+    ap.add_argument("--degridder-variant", default="auto", choices=["auto", "simt", "tensor", "fp64"])
     ap.add_argument("--no-other-configs", action="store_true",
                     help="skip the brief runs of configs 3, 4 and 5 that follow the config-2 headline")
     ap.add_argument("--e2e-batch", type=int, default=8192,

@@ -28,6 +28,12 @@ struct ProfRecord { int kind; cudaEvent_t a, b; };
 std::mutex g_prof_mu;
 bool g_prof_on = false;
 std::vector<ProfRecord> g_prof_pending;
+std::vector<cudaEvent_t> g_prof_pool;                // events of records already read, reused by later scopes
+
+bool prof_event(cudaEvent_t* e) {                    // g_prof_mu held
+  if (!g_prof_pool.empty()) { *e = g_prof_pool.back(); g_prof_pool.pop_back(); return true; }
+  return cudaEventCreate(e) == cudaSuccess;
+}
 
 struct ProfScope {
   cudaStream_t stream;
@@ -38,7 +44,7 @@ struct ProfScope {
     std::lock_guard<std::mutex> lock(g_prof_mu);
     on = g_prof_on;
     if (on) {
-      if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { on = false; return; }
+      if (!prof_event(&a) || !prof_event(&b)) { on = false; return; }
       cudaEventRecord(a, stream);
     }
   }
@@ -961,8 +967,9 @@ int idg_profile_read(double* ms_out, int64_t* launches_out) {
     if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, r.a, r.b);
     if (e == cudaSuccess) { ms_out[r.kind] += ms; launches_out[r.kind] += 1; }
     else if (first_err == cudaSuccess) first_err = e;
-    cudaEventDestroy(r.a);
-    cudaEventDestroy(r.b);
+    std::lock_guard<std::mutex> lock(g_prof_mu);
+    g_prof_pool.push_back(r.a);
+    g_prof_pool.push_back(r.b);
   }
   if (first_err != cudaSuccess) return cuda_fail(first_err, "idg_profile_read");
   return IDG_OK;

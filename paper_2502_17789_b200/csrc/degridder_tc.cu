@@ -282,7 +282,11 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
       // phasors and stores nothing: it only keeps the ring's barriers in step (its tensor-memory rows hold
       // stale finite-or-not values that no thread reads: MMA rows are independent).  The SIMT work is thus
       // padded to 32 visibilities, not 128 (low-occupancy tails).
+#ifdef IDG_DTC_NOTAIL
+      const bool warp_on = true;
+#else
       const bool warp_on = (t_base + tile_l) * kTileV + (uwarp & 3) * 32 < K;      // from warp-uniform values only
+#endif
       bool pending = false;                            // the ring's last slot is stored but not yet handed over
       auto drain = [&](int qq) {
         tc::mbar_wait(gbar + 16 * NA + 8 * (qq & 1), (qq >> 1) & 1);

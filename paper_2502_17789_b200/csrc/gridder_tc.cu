@@ -58,6 +58,20 @@ namespace {
 #ifndef IDG_TC_TF32
 #define IDG_TC_FP16 1                 // operand format: fp16 head + fp16 remainder (default) or split tf32
 #endif
+// fp16 operands (default): chunks of 16 channels (half the per-chunk ring / barrier bookkeeping of 8-channel chunks:
+// 6.32 against 5.82 pairs/clk/SM on config 2), a ring of 2 slots of 32 TMEM columns, accumulator groups of 6 chunks
+// (24 MMAs between drains, as with 12 chunks of 8).  Split tf32: chunks of 8, ring of 3, groups of 12.
+#ifdef IDG_TC_FP16
+#ifndef IDG_TC_KC
+#define IDG_TC_KC 16
+#endif
+#ifndef IDG_TC_DG
+#define IDG_TC_DG 6
+#endif
+#ifndef IDG_TC_NA
+#define IDG_TC_NA 2
+#endif
+#else
 #ifndef IDG_TC_KC
 #define IDG_TC_KC 8
 #endif
@@ -65,9 +79,6 @@ namespace {
 #define IDG_TC_DG 12
 #endif
 #ifndef IDG_TC_NA
-#ifdef IDG_TC_FP16
-#define IDG_TC_NA 4
-#else
 #define IDG_TC_NA 3
 #endif
 #endif
@@ -474,6 +485,14 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
         row_setup(r);
         uint32_t dk_addr = sdk_addr;
         int rig = 0, gin = 0;                          // revolutions in the current group, groups closed in this tile
+        // the A words of a chunk.  A half (8 channels) that lies wholly past the row's last channel is not
+        // generated: its words keep the previous chunk's (finite) values and meet zero rows of B.  The test is
+        // CTA-uniform (cc and nc are the subgrid's), so the SIMT work is padded to 8 channels, not to KC.
+        uint32_t hi[KC / 8][16];
+#pragma unroll
+        for (int h = 0; h < KC / 8; ++h)
+#pragma unroll
+          for (int w = 0; w < 16; ++w) hi[h][w] = 0u;
         for (int rev = 0; rev < nrev; ++rev) {
 #pragma unroll
           for (int s = 0; s < NA; ++s) {
@@ -482,7 +501,6 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
             // issued a whole hand-off / wait / store sequence ago
             if (s > 0) hand_off(gbar + 8 * (s - 1));
             else if (pending) hand_off(gbar + 8 * (NA - 1));
-            uint32_t hi[KC / 8][16];
             [[maybe_unused]] uint32_t lo[KC / 8][16];
 #ifdef IDG_TC_FP16
             if constexpr (ROT) {
@@ -491,6 +509,7 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
               // both components of e = (cos, sin) in one packed instruction each
 #pragma unroll
               for (int half = 0; half < KC / 8; ++half) {
+                if (half > 0 && cc + 8 * half >= nc) continue;
                 const float ph = fmaf(pa, tc::lds32(dk_addr + half * 32), pb);
                 float2 e;
                 __sincosf(ph, &e.y, &e.x);
@@ -512,6 +531,7 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
             if (valid) {
 #pragma unroll
               for (int half = 0; half < KC / 8; ++half) {
+                if (half > 0 && cc + 8 * half >= nc) continue;
                 const float4 dka = tc::lds128(dk_addr + half * 32);
                 const float4 dkb = tc::lds128(dk_addr + half * 32 + 16);
                 const float2 dk2[4] = {make_float2(dka.x, dka.y), make_float2(dka.z, dka.w),
@@ -647,7 +667,7 @@ cudaError_t launch_l(const SubgridJob& job, const float4* vis, float2* out, cuda
   constexpr int KC = IDG_TC_KC;
   const size_t dyn = static_cast<size_t>(std::min(job.max_nt * ((job.n_chan + KC - 1) / KC), kMaxBBytes / (KC * kVisBytes)) + IDG_TC_NA - 1) *
                      (KC * kVisBytes);
-  constexpr size_t kStaticAndReserved = 11 * 1024, kSmemPerSm = 227 * 1024;
+  constexpr size_t kStaticAndReserved = 12 * 1024, kSmemPerSm = 227 * 1024;
 #ifdef IDG_TC_NG
   return launch<L, IDG_TC_NG, KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
 #else

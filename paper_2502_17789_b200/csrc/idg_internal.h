@@ -16,7 +16,11 @@ constexpr int kMetaStride = 16;   // int32 per subgrid on the device: b,t0,nt,c0
 constexpr int kMetaConj = 1;      // flags bit 0: rows are used conjugated, (u,v,w) -> -(u,v,w), V -> V^dagger (R21); p,q already swapped
 constexpr int kTile = 32;         // adder tile edge in master-grid pixels
 constexpr int kAdderSegment = 128;   // subgrids one adder block walks; longer tile lists are split
-constexpr int kDegridTensorMin = 48;   // visibilities from which a subgrid takes the tensor-core degridder under AUTO
+// Visibilities from which a subgrid takes the tensor-core degridder under AUTO.  Measured on config 3 (occupancy
+// 1 ... 1536): sending the subgrids below 48 visibilities to the SIMT kernel cost 8 % of the launch (its lanes own 8
+// visibilities each, so a handful of visibilities leaves the block idle), while the tensor-core kernel's idle warps
+// cost nothing, so every subgrid takes the tensor-core kernel.
+constexpr int kDegridTensorMin = 1;
 constexpr int kSegStride = 6;     // int32 per adder segment: tile index, begin, end, k, n_seg, partial slot
 
 // tile -> subgrid lists for the atomic-free adder (one CSR per batch of subgrids).
