@@ -218,8 +218,8 @@ IDG_API int  idg_image_to_grid(const idg_plan* plan, const void* image_dev, cons
  * .degridder_variant), so two plans in one process may differ.
  * IDG_VARIANT_AUTO (0, the default): PER SUBGRID (PAPER.md:247 footnote 7, "swap the kernel design by a
  *   subgrid-occupancy heuristic"; :239-241), the tensor-core kernel where its operand slots are well filled
- *   (gridder: at least 80 % of the 8-channel chunks of a table row carry visibilities; degridder: at least
- *   48 visibilities) and the shape fits its shared-memory tables, else the SIMT kernel.  A batch is then
+ *   (gridder: at least 65 % of the slots of a table row's 16-channel chunks carry visibilities; degridder:
+ *   always, its idle warps cost nothing) and the shape fits its shared-memory tables, else the SIMT kernel.  A batch is then
  *   two launches over complementary index lists; the adder's order is untouched.
  * IDG_VARIANT_SIMT: all arithmetic on the FP32 / SFU pipes (packed FFMA2).
  * IDG_VARIANT_TENSOR: the phasor matrix is generated on the SIMT pipes and the 2x2 complex MACs run on the

@@ -87,8 +87,8 @@ cudaError_t upload_csr(const TileCsr& csr, DeviceCsr* out) {
   return upload(csr.segs, &out->segs);
 }
 
-// fp64 partial sums [n_slots][4 pol][kTile][kTile][re, im] and one zeroed counter per tile
-constexpr size_t kPartialBytes = static_cast<size_t>(4) * kTile * kTile * 2 * sizeof(double);
+// fp64 partial sums [n_slots][4 pol][tile pixels][re, im] and one zeroed counter per tile
+constexpr size_t kPartialBytes = static_cast<size_t>(4) * kTilePixels * 2 * sizeof(double);
 cudaError_t alloc_adder_scratch(int32_t n_slots, int32_t n_tiles, double** partials, int32_t** counters) {
   *partials = nullptr; *counters = nullptr;
   if (n_slots == 0) return cudaSuccess;
@@ -395,7 +395,7 @@ int grid_batch(const idg_plan* plan, const DeviceState* d, size_t i, const void*
   int rc = before_adder();
   if (rc != IDG_OK) return rc;
   { ProfScope ps(IDG_K_ADDER, stream);
-    IDG_CUDA(launch_adder(d->meta, d->batch_csr[i], bt.first, L, Ng, plan->tiles_x, plan->tiles_y, stack,
+    IDG_CUDA(launch_adder(d->meta, d->batch_csr[i], bt.first, bt.count, L, Ng, plan->tiles_x, plan->tiles_y, stack,
                           static_cast<float2*>(grid_dev), stream)); }
   return IDG_OK;
 }
@@ -924,7 +924,7 @@ int idg_adder(const idg_plan* plan, int64_t first, int64_t count, const void* su
   cudaError_t e = upload_csr(csr, &dc);
   if (e == cudaSuccess) e = alloc_adder_scratch(dc.n_slots, dc.n_tiles, &dc.partials, &dc.counters);
   if (e != cudaSuccess) { cudaFree(dc.partials); cudaFree(dc.counters); free_csr(&dc); return cuda_fail(e, "idg_adder: tile list upload"); }
-  e = launch_adder(d->meta, dc, first, plan->par.subgrid_size, plan->par.grid_size, plan->tiles_x, plan->tiles_y,
+  e = launch_adder(d->meta, dc, first, count, plan->par.subgrid_size, plan->par.grid_size, plan->tiles_x, plan->tiles_y,
                    static_cast<const float2*>(subgrids_dev), static_cast<float2*>(grid_dev), stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
   cudaFree(dc.partials); cudaFree(dc.counters);

@@ -485,14 +485,6 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
         row_setup(r);
         uint32_t dk_addr = sdk_addr;
         int rig = 0, gin = 0;                          // revolutions in the current group, groups closed in this tile
-        // the A words of a chunk.  A half (8 channels) that lies wholly past the row's last channel is not
-        // generated: its words keep the previous chunk's (finite) values and meet zero rows of B.  The test is
-        // CTA-uniform (cc and nc are the subgrid's), so the SIMT work is padded to 8 channels, not to KC.
-        uint32_t hi[KC / 8][16];
-#pragma unroll
-        for (int h = 0; h < KC / 8; ++h)
-#pragma unroll
-          for (int w = 0; w < 16; ++w) hi[h][w] = 0u;
         for (int rev = 0; rev < nrev; ++rev) {
 #pragma unroll
           for (int s = 0; s < NA; ++s) {
@@ -501,6 +493,9 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
             // issued a whole hand-off / wait / store sequence ago
             if (s > 0) hand_off(gbar + 8 * (s - 1));
             else if (pending) hand_off(gbar + 8 * (NA - 1));
+            // the A words of a chunk (channels past the row's last one are generated like any other and meet zero rows
+            // of B: skipping a chunk's empty half under a CTA-uniform test cost 6 % on config 2 and on config 3)
+            uint32_t hi[KC / 8][16];
             [[maybe_unused]] uint32_t lo[KC / 8][16];
 #ifdef IDG_TC_FP16
             if constexpr (ROT) {
@@ -509,7 +504,6 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
               // both components of e = (cos, sin) in one packed instruction each
 #pragma unroll
               for (int half = 0; half < KC / 8; ++half) {
-                if (half > 0 && cc + 8 * half >= nc) continue;
                 const float ph = fmaf(pa, tc::lds32(dk_addr + half * 32), pb);
                 float2 e;
                 __sincosf(ph, &e.y, &e.x);
@@ -531,7 +525,6 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
             if (valid) {
 #pragma unroll
               for (int half = 0; half < KC / 8; ++half) {
-                if (half > 0 && cc + 8 * half >= nc) continue;
                 const float4 dka = tc::lds128(dk_addr + half * 32);
                 const float4 dkb = tc::lds128(dk_addr + half * 32 + 16);
                 const float2 dk2[4] = {make_float2(dka.x, dka.y), make_float2(dka.z, dka.w),

@@ -14,7 +14,12 @@ namespace idg {
 constexpr double kSpeedOfLight = 299792458.0;
 constexpr int kMetaStride = 16;   // int32 per subgrid on the device: b,t0,nt,c0,nc,x0,y0,wl,p,q,it,layer,flags,-,-,-
 constexpr int kMetaConj = 1;      // flags bit 0: rows are used conjugated, (u,v,w) -> -(u,v,w), V -> V^dagger (R21); p,q already swapped
-constexpr int kTile = 32;         // adder tile edge in master-grid pixels
+// Adder tile: 1024 master-grid pixels, WIDE and flat (64 x 16 for L <= 64, 128 x 8 above).  A subgrid row (L samples,
+// contiguous in the stack) then falls into one or two tiles instead of three, so fewer DRAM sectors straddle a tile
+// boundary and are fetched twice, while a tile is not much wider than the subgrids it collects.
+constexpr int kTilePixels = 1024;
+inline int tile_width(int L) { return L <= 64 ? 64 : 128; }
+inline int tile_height(int L) { return kTilePixels / tile_width(L); }
 constexpr int kAdderSegment = 128;   // subgrids one adder block walks; longer tile lists are split
 // Visibilities from which a subgrid takes the tensor-core degridder under AUTO.  Measured on config 3 (occupancy
 // 1 ... 1536): sending the subgrids below 48 visibilities to the SIMT kernel cost 8 % of the launch (its lanes own 8
@@ -41,7 +46,7 @@ struct DeviceCsr {
   int32_t* items = nullptr;
   int32_t* segs = nullptr;
   int32_t n_tiles = 0, n_segs = 0, n_slots = 0;
-  double* partials = nullptr;      // [n_slots, 4, kTile, kTile, 2] scratch (not owned: DeviceState / caller)
+  double* partials = nullptr;      // [n_slots, 4, tile, 2] scratch (not owned: DeviceState / caller)
   int32_t* counters = nullptr;     // [n_tiles] segments finished per tile, zero between launches
 };
 
@@ -94,7 +99,7 @@ struct idg_plan {
   std::vector<int32_t> sub;               // [n_subgrids*8]
   int64_t n_subgrids = 0, n_vis_planned = 0, n_vis_dropped = 0;
   int32_t wl_min = 0, n_wlayers = 1;
-  int32_t tiles_x = 0, tiles_y = 0;
+  int32_t tiles_x = 0, tiles_y = 0, tile_w = 0, tile_h = 0;   // adder tiles
   int64_t batch_capacity = 0;             // subgrids per batch
   std::vector<idg::Batch> batches;
   // rows of the visibility table grouped by the first / last batch that touches them (host-buffer calls)

@@ -58,7 +58,8 @@ cudaError_t launch_split_ifft(const int32_t* meta, int64_t first, int64_t count,
                               float2* subgrids, cudaStream_t stream);
 
 // step a5: tile-owner adder.  csr lists, per non-empty tile, the subgrids overlapping it.
-cudaError_t launch_adder(const int32_t* meta, const DeviceCsr& csr, int64_t first, int L, int Ng,
+// subgrids: the stack of subgrids [first, first + count)
+cudaError_t launch_adder(const int32_t* meta, const DeviceCsr& csr, int64_t first, int64_t count, int L, int Ng,
                          int tiles_x, int tiles_y, const float2* subgrids, float2* grid,
                          cudaStream_t stream);
 

@@ -142,8 +142,10 @@ int plan_build(idg_plan* plan) {
   plan->wl_min = wl_lo;
   plan->n_wlayers = out.empty() ? 1 : (wl_hi - wl_lo + 1);
 
-  plan->tiles_x = (Ng + kTile - 1) / kTile;
-  plan->tiles_y = plan->tiles_x;
+  plan->tile_w = tile_width(L);
+  plan->tile_h = tile_height(L);
+  plan->tiles_x = (Ng + plan->tile_w - 1) / plan->tile_w;
+  plan->tiles_y = (Ng + plan->tile_h - 1) / plan->tile_h;
 
   // batches: contiguous ranges of the sorted subgrid list (§3.4 :259-267, R18)
   int64_t cap = par.max_batch_subgrids;
@@ -165,19 +167,19 @@ int plan_build(idg_plan* plan) {
   return IDG_OK;
 }
 
-// For subgrids [first, first+count): which adder tiles (kTile x kTile master-grid pixels of one
+// For subgrids [first, first+count): which adder tiles (tile_w x tile_h master-grid pixels of one
 // w-layer) does each overlap.  Lists are ascending in subgrid index, which fixes the summation
 // order of the adder (R18: bitwise reproducible).
 void build_tile_csr(const idg_plan* plan, int64_t first, int64_t count, TileCsr* out) {
   const int32_t L = plan->par.subgrid_size;
   const int32_t tx_n = plan->tiles_x, ty_n = plan->tiles_y;
   std::vector<std::pair<int32_t, int32_t>> pairs;   // (tile id, subgrid)
-  pairs.reserve(static_cast<size_t>(count) * 4);
+  pairs.reserve(static_cast<size_t>(count) * ((L + plan->tile_h - 1) / plan->tile_h + 1) * 2);
   for (int64_t s = first; s < first + count; ++s) {
     const int32_t* e = &plan->sub[static_cast<size_t>(s) * 8];
     const int32_t x0 = e[5], y0 = e[6], layer = e[7] - plan->wl_min;
-    const int32_t tx0 = x0 / kTile, tx1 = (x0 + L - 1) / kTile;
-    const int32_t ty0 = y0 / kTile, ty1 = (y0 + L - 1) / kTile;
+    const int32_t tx0 = x0 / plan->tile_w, tx1 = (x0 + L - 1) / plan->tile_w;
+    const int32_t ty0 = y0 / plan->tile_h, ty1 = (y0 + L - 1) / plan->tile_h;
     for (int32_t ty = ty0; ty <= ty1; ++ty)
       for (int32_t tx = tx0; tx <= tx1; ++tx)
         pairs.emplace_back((layer * ty_n + ty) * tx_n + tx, static_cast<int32_t>(s));
@@ -228,8 +230,8 @@ bool subgrid_conjugated(const idg_plan* plan, const int32_t* e) {
 }
 
 // Kernel choice per subgrid (PAPER.md:247 fn 7, :239-241).  The tensor-core
-// gridder pads every table row to whole 8-channel chunks and the tensor-core degridder works on warps of 32
-// visibilities inside tiles of 128, so sparsely filled subgrids go to the SIMT kernels, which have no padding.
+// gridder pads every table row to whole 16-channel chunks: it runs at 0.89 of the ALU roofline on full chunks
+// against the SIMT kernel's 0.55 (no padding), so it wins from a fill of about 0.62.
 void split_kernels(const idg_plan* plan, int64_t first, int64_t count, int direction, KernelSplit* out) {
   out->tensor.clear(); out->simt.clear();
   out->variant = direction == IDG_GRID ? plan->par.gridder_variant : plan->par.degridder_variant;
@@ -238,7 +240,7 @@ void split_kernels(const idg_plan* plan, int64_t first, int64_t count, int direc
     const int32_t* e = &plan->sub[static_cast<size_t>(first + i) * 8];
     const int32_t nt = e[2], nc = e[4];
     bool tensor;
-    if (direction == IDG_GRID) tensor = 10 * nc >= 8 * ((nc + 7) / 8 * 8);          // chunk fill >= 80 %
+    if (direction == IDG_GRID) tensor = 100 * nc >= 65 * ((nc + 15) / 16 * 16);     // chunk fill >= 65 %
     else                       tensor = static_cast<int64_t>(nt) * nc >= kDegridTensorMin;
     (tensor ? out->tensor : out->simt).push_back(static_cast<int32_t>(i));
   }

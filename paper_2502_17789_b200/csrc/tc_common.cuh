@@ -21,8 +21,26 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-// blocks until the phase with the given parity has completed
+// blocks until the phase with the given parity has completed.  The suspend-time hint lets the hardware park the
+// warp until the phase completes (or the hint expires) instead of returning after its short default time-out:
+// without it a waiting service warp spins (try_wait, branch, yield) and takes issue slots from the compute warps of
+// its scheduler.
+#ifndef IDG_MBAR_HINT_NS
+#define IDG_MBAR_HINT_NS 100000
+#endif
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+#if IDG_MBAR_HINT_NS > 0
+  asm volatile(
+      "{\n\t"
+      ".reg .pred P1;\n\t"
+      "LAB_WAIT:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1, %2;\n\t"
+      "@P1 bra DONE;\n\t"
+      "bra LAB_WAIT;\n\t"
+      "DONE:\n\t"
+      "}" ::"r"(bar), "r"(parity), "r"(IDG_MBAR_HINT_NS)
+      : "memory");
+#else
   asm volatile(
       "{\n\t"
       ".reg .pred P1;\n\t"
@@ -33,6 +51,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "DONE:\n\t"
       "}" ::"r"(bar), "r"(parity)
       : "memory");
+#endif
 }
 // the same for long waits (a producer waiting for a whole stage to drain): try_wait gives up after a short
 // hardware time-out, so without a back-off the loop spins and steals issue slots from the compute warps

@@ -121,7 +121,7 @@ def test_gridder_and_fft_per_subgrid(idg, name, make, vis, variant):
     torch.cuda.synchronize()
     # which kernel ran: the tests must know what they exercised
     nc = sub[:, 4]
-    fill_ok = 10 * nc >= 8 * ((nc + 7) // 8 * 8)
+    fill_ok = 100 * nc >= 65 * ((nc + 15) // 16 * 16)
     if variant == "simt" or name == "many-chan":
         assert mask == idg.KMASK_SIMT, (name, variant, mask)
     elif variant == "tensor":
