@@ -27,6 +27,14 @@
 // 1.8e-6 with tf32 operands (48 MMAs).  Halving the bytes stored per pair is also why it is faster (the
 // tensor-memory stores cost 20 % of the tf32 kernel's time): 5.45 against 5.19 pairs/clk/SM on config 2.
 //
+// Phasors by rotation (round 2, template parameter ROT; uniformly spaced channels): the phase is linear in the channel,
+// so per 8 channels ONE __sincosf seeds e = (cos, sin) and 7 steps of d += -4 sin^2(delta/2) e, e += d (one packed FFMA2
+// and one packed FADD2 each) give the rest; delta = pa * dkappa per (row, pixel), its 1 - cos and sin from Taylor series
+// at delta / 4 plus two angle doublings (relative accuracy: a rotor error grows linearly along the chain).  MUFU per pair
+// 2 -> 0.25.  Chunks are 16 channels (KC) with fp16 operands: half the per-chunk bookkeeping, one tcgen05.st.x32, four
+// K = 16 MMAs, a ring of 2 slots, accumulator groups of 6 chunks.  6.32 pairs/clk/SM on config 2 (0.89 of the ALU
+// roofline) against 5.38 for the round-1 kernel.
+//
 // One CTA per subgrid: NG groups of 128 compute threads plus one service warp per group; NG = 1, 2 or 4
 // chosen at launch so that 4 / NG CTAs share an SM (see launch_l).
 //   all threads      stage the B operand of the subgrid's visibilities ONCE in shared memory (heads
@@ -34,7 +42,7 @@
 //                    Subgrids with more visibilities than fit are processed in segments of whole table
 //                    rows; partial sums then pass through the output buffer.
 //   compute group    owns one tile of 128 pixels per round (thread = pixel = MMA row = TMEM lane).
-//                    Per chunk of <= KC channels of one table row: sincos -> head/remainder ->
+//                    Per chunk of <= KC channels of one table row: seed + rotations (or sincos) -> head/remainder ->
 //                    tcgen05.st into the group's A ring slot.  The hand-off of chunk g (wait::st,
 //                    fence, mbarrier arrive) is issued after the arithmetic of chunk g+1, so the
 //                    store latency is hidden.  Accumulators are drained one group of DG chunks late,
