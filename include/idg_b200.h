@@ -240,11 +240,13 @@ IDG_API int  idg_image_to_grid(const idg_plan* plan, const void* image_dev, cons
 
 /* Which kernels the direct-sum step `kind` (IDG_K_GRIDDER or IDG_K_DEGRIDDER) has launched in this process
  * since the last reset, as a bit mask: bit 0 SIMT, bit 1 / 2 / 4 tensor-core with 1 / 2 / 4 compute groups
- * per CTA (the gridder picks by shared-memory fit; the degridder always runs 2), bit 8 fp64.  reset != 0
+ * per CTA (the gridder picks by shared-memory fit; the degridder always runs 2), bit 8 fp64, bit 9 the tensor-core
+ * gridder with phasor rotation along the channel axis (uniformly spaced channels; otherwise one sincos per pair).  reset != 0
  * clears the mask after reading.  For the tests, which must know what they exercised. */
 #define IDG_KMASK_SIMT   (1 << 0)
 #define IDG_KMASK_TC(ng) (1 << (ng))
 #define IDG_KMASK_FP64   (1 << 8)
+#define IDG_KMASK_ROT    (1 << 9)
 IDG_API int  idg_kernel_config_mask(int kind, int reset);
 
 /* fp64 stage calls: the two direct sums with their A-term /

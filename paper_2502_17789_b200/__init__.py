@@ -167,7 +167,7 @@ class PlanCounts:
 
 
 VARIANT_AUTO, VARIANT_SIMT, VARIANT_TENSOR, VARIANT_FP64 = 0, 1, 2, 3
-KMASK_SIMT, KMASK_FP64 = 1 << 0, 1 << 8
+KMASK_SIMT, KMASK_FP64, KMASK_ROT = 1 << 0, 1 << 8, 1 << 9
 
 
 def kmask_tc(ng: int) -> int:

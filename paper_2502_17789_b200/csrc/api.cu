@@ -206,6 +206,7 @@ SubgridJob make_job(const idg_plan* plan, const DeviceState* d, int64_t first, i
   j.index = nullptr;
   j.power_norm = plan->par.power_norm;
   j.dkappa = plan->dkappa;
+  j.dkappa_f = static_cast<float>(plan->dkappa);
   j.first = first; j.count = count;
   j.subgrid_size = plan->par.subgrid_size; j.grid_size = plan->par.grid_size;
   j.n_times = plan->par.n_times; j.n_chan = plan->par.n_chan; j.n_intervals = plan->n_intervals;

@@ -242,7 +242,7 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
   const float4* __restrict__ aq = job.aterms + (static_cast<int64_t>(sq) * job.n_intervals + it) * (L * L * 2);
   float2* o = out + sg * 4 * L * L;
   const uint32_t sdk_addr = tc::opaque(tc::smem_u32(&sdk[0]));
-  [[maybe_unused]] const float dkf = static_cast<float>(job.dkappa);   // channel spacing in kappa (ROT)
+  const uint32_t srow_addr = tc::opaque(tc::smem_u32(&srow[0]));
 
   for (int seg = 0; seg < nseg; ++seg) {
     const int r_begin = seg * rows_per_seg, r_end = min(nt, r_begin + rows_per_seg);
@@ -460,12 +460,16 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
         [[maybe_unused]] float2 nk2 = make_float2(0.f, 0.f);     // (-2 kh, -2 kh) = -4 sin^2(delta / 2)
         [[maybe_unused]] float kh = 0.f, sg = 0.f;
         auto row_setup = [&](int r) {
-          const RowDataTc rd = srow[r];
+          // the row's 32 bytes as two 128-bit loads from an address kept in a register
+          const float4 ra = tc::lds128(srow_addr + r * 32), rb = tc::lds128(srow_addr + r * 32 + 16);
+          RowDataTc rd;
+          rd.alpha_fix = __float_as_int(ra.x); rd.beta_fix = __float_as_int(ra.y); rd.gamma = ra.z; rd.us = ra.w;
+          rd.vs = rb.x; rd.ws = rb.y; rd.dmax = rb.z;
           pa = fmaf(rd.vs, static_cast<float>(iy), fmaf(rd.ws, np, rd.us * static_cast<float>(ix)));
           const int32_t bf = rd.alpha_fix * ix + rd.beta_fix * iy;                  // wraps: exact mod 1 cycle
           pb = fmaf(rd.gamma, np, static_cast<float>(bf) * 1.4629180792671596e-9f);   // 2 pi / 2^32
           if constexpr (ROT) {
-            const float delta = pa * dkf;
+            const float delta = pa * job.dkappa_f;
             if (rd.dmax < 3.0f) {                        // CTA-uniform
               const float x = 0.25f * delta, t = x * x;
               // sin x = x (1 - t/6 + t^2/120 - t^3/5040 + t^4/362880), 1 - cos x = t (1/2 - t/24 + t^2/720 - t^3/40320)
@@ -516,15 +520,15 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
                 float2 e;
                 __sincosf(ph, &e.y, &e.x);
                 float2 d = make_float2(fmaf(-kh, e.x, -sg * e.y), fmaf(-kh, e.y, sg * e.x));
-                const float2 m1 = make_float2(-1.f, -1.f);
 #pragma unroll
                 for (int j = 0; j < 8; ++j) {
                   if (j == 1) e = __fadd2_rn(e, d);
                   if (j > 1) { d = ffma2(e, nk2, d); e = __fadd2_rn(e, d); }
                   const __half2 q = __floats2half2_rn(e.x, e.y);
-                  const float2 l = ffma2(__half22float2(q), m1, e);
+                  const uint32_t qw = *reinterpret_cast<const uint32_t*>(&q);
+                  const float2 l = tc::sub_half2(e, qw);
                   const __half2 rr = __floats2half2_rn(l.x, l.y);
-                  hi[half][j] = *reinterpret_cast<const uint32_t*>(&q);
+                  hi[half][j] = qw;
                   hi[half][8 + j] = *reinterpret_cast<const uint32_t*>(&rr);
                 }
               }
@@ -548,9 +552,8 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
 #ifdef IDG_TC_FP16
                   // (cos, sin) -> fp16 head pair and fp16 remainder pair, one 32-bit word each
                   const __half2 q0 = __floats2half2_rn(e0.x, e0.y), q1 = __floats2half2_rn(e1.x, e1.y);
-                  const float2 f0 = __half22float2(q0), f1 = __half22float2(q1);
-                  const float2 m1 = make_float2(-1.f, -1.f);
-                  const float2 l0 = ffma2(f0, m1, e0), l1 = ffma2(f1, m1, e1);
+                  const float2 l0 = tc::sub_half2(e0, *reinterpret_cast<const uint32_t*>(&q0));
+                  const float2 l1 = tc::sub_half2(e1, *reinterpret_cast<const uint32_t*>(&q1));
                   const __half2 r0 = __floats2half2_rn(l0.x, l0.y), r1 = __floats2half2_rn(l1.x, l1.y);
                   hi[half][2 * j2] = *reinterpret_cast<const uint32_t*>(&q0);
                   hi[half][2 * j2 + 1] = *reinterpret_cast<const uint32_t*>(&q1);
@@ -646,7 +649,7 @@ cudaError_t launch_rot(const SubgridJob& job, const float4* vis, float2* out, cu
   if (e != cudaSuccess) return e;
   kernel<<<static_cast<unsigned>(job.count), NG * kTileM + NG * 32, dyn, stream>>>(job, vis, out, cap_chunks);
   count_launch();
-  note_kernel(IDG_K_GRIDDER, IDG_KMASK_TC(NG));
+  note_kernel(IDG_K_GRIDDER, IDG_KMASK_TC(NG) | (ROT ? IDG_KMASK_ROT : 0));
   return cudaGetLastError();
 }
 

@@ -27,6 +27,7 @@ struct SubgridJob {
   double image_size;        // S
   double w_step;
   double dkappa;            // kappa[c + 1] - kappa[c] when the channels are uniformly spaced, else 0
+  float dkappa_f;           // the same rounded to fp32 (a constant-bank operand of the rotating gridder)
   int32_t power_norm;       // imaging: divide the sandwich by || M_p M_q^H ||_F per pixel (R22)
 };
 

@@ -210,6 +210,21 @@ __device__ __forceinline__ float4 lds128(uint32_t addr) {
   asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
   return v;
 }
+// e - float(h) for the two halves of a packed half2 h2: one mixed-precision FMA each (fma.rn.f32.f16, SASS FHFMA,
+// half x half + float -> float), exact because h is e rounded to fp16.  Replaces two half -> float conversions and
+// a packed subtraction.
+__device__ __forceinline__ float2 sub_half2(float2 e, uint32_t h2) {
+  float x, y;
+  asm("{\n\t"
+      ".reg .b16 lo, hi;\n\t"
+      "mov.b32 {lo, hi}, %2;\n\t"
+      "fma.rn.f32.f16 %0, lo, %5, %3;\n\t"
+      "fma.rn.f32.f16 %1, hi, %5, %4;\n\t"
+      "}"
+      : "=f"(x), "=f"(y)
+      : "r"(h2), "f"(e.x), "f"(e.y), "h"(static_cast<unsigned short>(0xBC00)));   // -1 in fp16
+  return make_float2(x, y);
+}
 __device__ __forceinline__ float lds32(uint32_t addr) {
   float v;
   asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));

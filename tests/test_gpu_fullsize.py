@@ -124,7 +124,7 @@ def test_full_size_config3_sampled(idg):
     idg.kernel_config_mask("gridder", reset=True)
     idg.kernel_config_mask("degridder", reset=True)
     d_grid = grid_twice(idg, plan, d_vis, d_at, d_tp, cnt, Ng, ws)
-    assert idg.kernel_config_mask("gridder") == idg.KMASK_SIMT | idg.kmask_tc(2)
+    assert idg.kernel_config_mask("gridder") == idg.KMASK_SIMT | idg.kmask_tc(2) | idg.KMASK_ROT
     scale = max(float(torch.abs(d_grid[k]).max()) for k in range(cnt.n_wlayers))
     vis = OnDevice(d_vis)
     # pixels of the layers either side of w = 0 and of the outermost layers

@@ -69,6 +69,9 @@ CASES = [
      "hash"),
     ("L128-ng2", lambda: synth.scaled(synth.get_config(2), n_stations=6, n_times=8, n_chan=96, subgrid_size=128,
                                       padding=24), "hash"),
+    # channel steps of up to 4 rad of phase at the subgrid's edge: the rotating gridder takes its rotor from the accurate
+    # sincosf on such rows instead of the small-angle series
+    ("big-step", lambda: synth.scaled(synth.get_config(1), n_stations=6, n_times=8, n_chan=16, chan_width_hz=2.2e6), "hash"),
     # the two further subgrid sizes of PAPER.md Fig. 7 :363-369
     ("L48", lambda: synth.scaled(synth.get_config(1), n_stations=7, n_times=16, n_chan=16, subgrid_size=48,
                                  padding=10), "hash"),
@@ -117,6 +120,7 @@ def test_gridder_and_fft_per_subgrid(idg, name, make, vis, variant):
     idg.kernel_config_mask("gridder", reset=True)
     idg.grid_subgrids(plan, 0, n, d_vis, d_at, d_tp, out_img, stage=idg.STAGE_GRIDDER)
     mask = idg.kernel_config_mask("gridder", reset=True)
+    rot, mask = bool(mask & idg.KMASK_ROT), mask & ~idg.KMASK_ROT
     idg.grid_subgrids(plan, 0, n, d_vis, d_at, d_tp, out_uv, stage=idg.STAGE_FFT)
     torch.cuda.synchronize()
     # which kernel ran: the tests must know what they exercised
@@ -126,6 +130,7 @@ def test_gridder_and_fft_per_subgrid(idg, name, make, vis, variant):
         assert mask == idg.KMASK_SIMT, (name, variant, mask)
     elif variant == "tensor":
         assert mask & ~idg.KMASK_SIMT and not mask & idg.KMASK_SIMT, (name, variant, mask)
+        assert rot, "uniformly spaced channels: the rotating kernel must have run"
         if name in EXPECT_NG:
             assert mask == idg.kmask_tc(EXPECT_NG[name]), (name, mask)
     else:
@@ -671,3 +676,29 @@ def test_fp64_direct_sums(idg, name, make):
                                       orc.aterm_taper(np.moveaxis(S[s].astype(np.complex64).astype(np.complex128), 0, 2),
                                                       Mp, Mq, obs.taper))
         assert nerr(h32[r0:r0 + nt, c0:c0 + nc], ref32) <= 1e-7, (name, s)
+
+
+@pytest.mark.parametrize("variant", ["tensor", "auto"])
+def test_nonuniform_channels(idg, variant):
+    """Channels that are NOT uniformly spaced (PAPER.md:196 only asks for ascending order): the planner then sets no
+    channel step and the tensor-core gridder runs its one-sincos-per-pair form instead of the rotation."""
+    cfg = synth.scaled(synth.get_config(2), n_stations=8, n_times=16)
+    obs = synth.make_observation(cfg, vis="hash")
+    rng = np.random.default_rng(31)
+    obs.freqs = obs.freqs + rng.uniform(-0.3, 0.3, cfg.n_chan) * cfg.chan_width_hz
+    assert np.all(np.diff(obs.freqs) > 0)
+    par = oracle_params(cfg)
+    plan = idg.plan_from_config(cfg, obs.uvw, obs.freqs, obs.baselines, gridder_variant=VAR[variant])
+    sub = plan.export()
+    ref_sub, _ = orc.plan(par, obs.uvw, obs.freqs, cfg.n_baselines)
+    assert np.array_equal(sub, ref_sub)
+    L, n = cfg.subgrid_size, len(sub)
+    out = torch.zeros((n, 4, L, L), dtype=torch.complex64, device=DEV)
+    idg.kernel_config_mask("gridder", reset=True)
+    idg.grid_subgrids(plan, 0, n, dev(obs.vis), dev(obs.aterms), dev(obs.taper), out, stage=idg.STAGE_GRIDDER)
+    mask = idg.kernel_config_mask("gridder", reset=True)
+    assert mask == idg.kmask_tc(1), mask                  # tensor-core, one group per CTA, no rotation bit
+    g = out.cpu().numpy()
+    for s in sample_subgrids(sub, 8):
+        Sp, _ = orc.grid_subgrid(par, sub[s], obs.uvw, obs.freqs, obs.vis, obs.baselines, obs.aterms, obs.taper)
+        assert nerr(np.moveaxis(g[s], 0, 2), Sp) <= TOL
