@@ -539,7 +539,7 @@ def run_ours(args):
 def ncu_traffic(kernel, cfg, n_subgrids, launches_per_step):
     """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/), scaled from the
     captured launch to this run's average launch; None when there is no capture for this workload."""
-    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "dram_traffic_r02b.csv")
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "dram_traffic_r02c.csv")
     if cfg.config_id != 2 or not os.path.exists(path) or not launches_per_step:
         return None
     with open(path) as f:

@@ -230,8 +230,8 @@ bool subgrid_conjugated(const idg_plan* plan, const int32_t* e) {
 }
 
 // Kernel choice per subgrid (PAPER.md:247 fn 7, :239-241).  The tensor-core
-// gridder pads every table row to whole 16-channel chunks: it runs at 0.89 of the ALU roofline on full chunks
-// against the SIMT kernel's 0.55 (no padding), so it wins from a fill of about 0.62.
+// gridder pads every table row to whole 16-channel chunks: it runs at 0.96 of the ALU roofline on full chunks
+// against the SIMT kernel's 0.55 (no padding), so it wins from a fill of about 0.6.
 void split_kernels(const idg_plan* plan, int64_t first, int64_t count, int direction, KernelSplit* out) {
   out->tensor.clear(); out->simt.clear();
   out->variant = direction == IDG_GRID ? plan->par.gridder_variant : plan->par.degridder_variant;
