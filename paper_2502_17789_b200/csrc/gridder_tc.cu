@@ -455,8 +455,8 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
         // ROT: the phase is linear in the channel, phi(c + 1) = phi(c) + delta with delta = pa * dkappa per (row,
         // pixel), so e(c + 1) = e(c) rot, rot = exp(i delta) (the per-row precomputation, one step
         // further).  Kept as kh = 1 - cos(delta) and sg = sin(delta), both to RELATIVE fp32 accuracy (a rotor error
-        // grows linearly along the chain): Taylor series at delta / 4 and two angle doublings for |delta| < 3,
-        // the accurate sincosf beyond (short rows of long baselines).
+        // grows linearly along the chain): Taylor series at delta for |delta| < 0.5, at delta / 4 with two angle
+        // doublings for |delta| < 3, the accurate sincosf beyond (short rows of long baselines).
         [[maybe_unused]] float2 nk2 = make_float2(0.f, 0.f);     // (-2 kh, -2 kh) = -4 sin^2(delta / 2)
         [[maybe_unused]] float kh = 0.f, sg = 0.f;
         auto row_setup = [&](int r) {
@@ -470,7 +470,16 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
           pb = fmaf(rd.gamma, np, static_cast<float>(bf) * 1.4629180792671596e-9f);   // 2 pi / 2^32
           if constexpr (ROT) {
             const float delta = pa * job.dkappa_f;
-            if (rd.dmax < 3.0f) {                        // CTA-uniform
+            if (rd.dmax < 0.5f) {                        // CTA-uniform: the series at delta itself (error < 5e-9 relative)
+              const float t = delta * delta;
+              float s1 = fmaf(t, -1.9841270e-4f, 8.3333333e-3f);
+              s1 = fmaf(t, s1, -1.6666667e-1f);
+              sg = fmaf(delta * t, s1, delta);
+              float k1 = fmaf(t, -2.4801587e-5f, 1.3888889e-3f);
+              k1 = fmaf(t, k1, -4.1666667e-2f);
+              k1 = fmaf(t, k1, 0.5f);
+              kh = k1 * t;
+            } else if (rd.dmax < 3.0f) {
               const float x = 0.25f * delta, t = x * x;
               // sin x = x (1 - t/6 + t^2/120 - t^3/5040 + t^4/362880), 1 - cos x = t (1/2 - t/24 + t^2/720 - t^3/40320)
               float s1 = fmaf(t, 2.7557319e-6f, -1.9841270e-4f);
