@@ -27,7 +27,7 @@ SYMBOLS = (
     "idg_grid_subgrids", "idg_degrid_subgrids", "idg_subgrid_fft", "idg_adder", "idg_splitter",
     "idg_closure_workspace_bytes", "idg_grid_to_image", "idg_image_to_grid",
     "idg_grid_subgrids_f64", "idg_degrid_subgrids_f64", "idg_power_norm_average",
-    "idg_profile_enable", "idg_profile_read", "idg_kernel_config_mask",
+    "idg_profile_enable", "idg_profile_read", "idg_kernel_config_mask", "idg_plan_kernel_split",
     "idg_measure_alu_peaks", "idg_launch_count", "idg_last_error", "idg_version",
 )
 KERNEL_KINDS = ("gridder", "fft", "adder", "splitter", "ifft", "degridder")
@@ -107,6 +107,8 @@ def load_library() -> ctypes.CDLL:
     lib.idg_profile_enable.restype = ctypes.c_int
     lib.idg_profile_read.argtypes = [vp, vp]
     lib.idg_profile_read.restype = ctypes.c_int
+    lib.idg_plan_kernel_split.argtypes = [vp, ctypes.c_int, ctypes.POINTER(i64), ctypes.POINTER(i64)]
+    lib.idg_plan_kernel_split.restype = ctypes.c_int
     lib.idg_kernel_config_mask.argtypes = [ctypes.c_int, ctypes.c_int]
     lib.idg_kernel_config_mask.restype = ctypes.c_int
     lib.idg_grid_subgrids_f64.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
@@ -240,6 +242,13 @@ class Plan:
         _check(load_library().idg_host_traffic_bytes(self._h, direction, ctypes.byref(up), ctypes.byref(down)),
                "idg_host_traffic_bytes")
         return int(up.value), int(down.value)
+
+    def kernel_split(self, direction=IDG_GRID):
+        """(tensor-core, SIMT) subgrid counts of a direction under the plan's kernel variant."""
+        nt, ns = ctypes.c_int64(), ctypes.c_int64()
+        _check(load_library().idg_plan_kernel_split(self._h, direction, ctypes.byref(nt), ctypes.byref(ns)),
+               "idg_plan_kernel_split")
+        return int(nt.value), int(ns.value)
 
     def closure_workspace_bytes(self) -> int:
         return int(load_library().idg_closure_workspace_bytes(self._h))

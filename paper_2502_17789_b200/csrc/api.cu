@@ -976,6 +976,20 @@ int idg_profile_read(double* ms_out, int64_t* launches_out) {
   return IDG_OK;
 }
 
+int idg_plan_kernel_split(const idg_plan* plan, int direction, int64_t* n_tensor, int64_t* n_simt) {
+  if (!plan || (direction != IDG_GRID && direction != IDG_DEGRID)) { set_error("idg_plan_kernel_split: bad argument"); return IDG_EINVAL; }
+  int64_t nt = 0, ns = 0;
+  for (const Batch& bt : plan->batches) {
+    const KernelSplit& sp = direction == IDG_GRID ? bt.grid_split : bt.degrid_split;
+    if (sp.variant == IDG_VARIANT_AUTO) { nt += static_cast<int64_t>(sp.tensor.size()); ns += static_cast<int64_t>(sp.simt.size()); }
+    else if (sp.variant == IDG_VARIANT_TENSOR) nt += bt.count;
+    else ns += bt.count;
+  }
+  if (n_tensor) *n_tensor = nt;
+  if (n_simt) *n_simt = ns;
+  return IDG_OK;
+}
+
 int idg_kernel_config_mask(int kind, int reset) {
   if (kind != IDG_K_GRIDDER && kind != IDG_K_DEGRIDDER) { set_error("idg_kernel_config_mask: bad kind"); return IDG_EINVAL; }
   return reset ? g_kmask[kind].exchange(0) : g_kmask[kind].load();

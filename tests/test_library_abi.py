@@ -87,6 +87,43 @@ def test_plan_positive_w_bit_exact_vs_oracle(idg, name, make):
             assert np.all(sg == sg[0]) or np.all(w[b, t0:t0 + nt] >= 0) or np.all(w[b, t0:t0 + nt] < 0)
 
 
+def test_config3_full_size_layers_halve_with_positive_w(idg):
+    """BASELINE.json configs[2] at full size (host planner only): 10 signed w-layers of 50 lambda become 5 with
+    positive_w (PAPER.md:178 fn 4: the conjugation 'halves the number of w-layers'), with the same subgrid count and
+    every visibility still planned."""
+    cfg = synth.get_config(3)
+    obs = synth.make_observation(cfg, vis=None, with_aterms=False)
+    signed = _plan(idg, cfg, obs).counts()
+    pos = _plan(idg, cfg, obs, positive_w=True).counts()
+    assert (signed.n_wlayers, signed.wl_min) == (10, -5) and (pos.n_wlayers, pos.wl_min) == (5, 0)
+    assert signed.n_vis_planned == pos.n_vis_planned == cfg.n_vis and pos.n_vis_dropped == 0
+    assert signed.n_subgrids == pos.n_subgrids == 517794
+
+
+def test_kernel_choice_per_subgrid(idg):
+    """PAPER.md:247 (fn 7): under AUTO the gridder's subgrids go to the tensor-core kernel
+    where at least 65 % of the slots of their 16-channel chunks are filled, to the SIMT kernel otherwise; every
+    subgrid takes the tensor-core degridder; forced variants take everything; batches do not change the split."""
+    cfg = synth.scaled(synth.get_config(3), n_stations=6, n_times=8)         # 1 ... 384 channels per subgrid
+    obs = synth.make_observation(cfg, vis=None, with_aterms=False)
+    plan = _plan(idg, cfg, obs)
+    sub = plan.export()
+    nc = sub[:, 4].astype(np.int64)
+    want_tc = int((100 * nc >= 65 * ((nc + 15) // 16 * 16)).sum())
+    assert 0 < want_tc < len(sub), "case must mix both kinds"
+    assert plan.kernel_split(idg.IDG_GRID) == (want_tc, len(sub) - want_tc)
+    assert plan.kernel_split(idg.IDG_DEGRID) == (len(sub), 0)
+    assert _plan(idg, cfg, obs, max_batch_subgrids=7).kernel_split(idg.IDG_GRID) == (want_tc, len(sub) - want_tc)
+    assert _plan(idg, cfg, obs, gridder_variant=idg.VARIANT_SIMT).kernel_split(idg.IDG_GRID) == (0, len(sub))
+    assert _plan(idg, cfg, obs, gridder_variant=idg.VARIANT_TENSOR).kernel_split(idg.IDG_GRID) == (len(sub), 0)
+    # config 1: 4 channels per row -> all SIMT; config 2: 32 -> all tensor-core
+    for cid, all_tc in ((1, False), (2, True)):
+        c = synth.scaled(synth.get_config(cid), n_stations=8)
+        o = synth.make_observation(c, vis=None, with_aterms=False)
+        nt, ns = _plan(idg, c, o).kernel_split(idg.IDG_GRID)
+        assert (ns == 0) if all_tc else (nt == 0)
+
+
 def test_workspace_follows_batch_capacity(idg):
     cfg = synth.get_config(1)
     obs = synth.make_observation(cfg, vis=None, with_aterms=False)
