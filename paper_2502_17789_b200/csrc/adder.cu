@@ -266,6 +266,8 @@ cudaError_t launch_adder(const int32_t* meta, const DeviceCsr& csr, int64_t firs
                          int tiles_y, const float2* subgrids, float2* grid, cudaStream_t stream) {
   if (csr.n_segs == 0) return cudaSuccess;
   if (csr.n_slots > 0 && (!csr.partials || !csr.counters)) return cudaErrorInvalidValue;
+  // the tensor map wants a 16-byte aligned base (include/idg_b200.h asks that of every device pointer)
+  if (reinterpret_cast<uintptr_t>(subgrids) & 15) return cudaErrorMisalignedAddress;
   const int W = tile_width(L), H = tile_height(L);
   CUtensorMap map;
   cudaError_t e = stack_tensor_map(subgrids, L, count, W, H, &map);
