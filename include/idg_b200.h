@@ -273,6 +273,41 @@ IDG_API int  idg_degrid_subgrids_f64(const idg_plan* plan, int64_t first, int64_
 IDG_API int  idg_power_norm_average(const idg_plan* plan, const void* aterms_dev, double* avg_dev,
                             void* cuda_stream);
 
+/* ---- the same average for callers that cannot allocate device memory ------------------------------------
+ * idg_power_norm_average allocates (and frees) three device buffers per call.  Two kinds of caller cannot
+ * live with that: one whose own pool took the whole device at start-up (master grids fill the card,
+ * PAPER.md:399-405), where a raw cudaMalloc fails although the pool has room; and one that prepares the
+ * correction while gridding batches run on other streams, because cudaMalloc / cudaFree synchronise the whole
+ * device and stall them.  idg_power_norm_average_static calls no cudaMalloc, no cudaFree and no allocating
+ * library routine, takes no plan (so it never triggers the plan's metadata upload) and does not synchronise:
+ * the two kernels are enqueued on cuda_stream and avg_dev is valid when they have run.
+ *
+ * Its scratch (64 x L x L fp64 partial sums) is an array built into the library:
+ * 64 x 96 x 96 x 8 B = 4.5 MiB of every GPU that loads the library, until the process exits.  Hence
+ *   - subgrid_size > IDG_STATIC_MAX_SUBGRID_SIZE (96) is refused with IDG_EUNSUPPORTED and a message naming
+ *     the limit (L = 128 and 160 need idg_power_norm_average);
+ *   - all calls on one device share that array.  It needs no clearing (each call overwrites what it reads)
+ *     and keeps the last call's partial sums, but two calls that overlap on the GPU -- different streams,
+ *     different host threads, different plans -- race on it and both results are garbage.  Order them.
+ *   - the first call on each device looks up the array's device address (one cudaGetSymbolAddress, with that
+ *     device current).  Make that first call during set-up, before any stream capture begins.
+ *
+ * The caller passes everything else, already on the device (16-byte aligned):
+ *   aterms_dev  [n_stations, n_intervals, L, L, 2, 2] complex64, as for idg_grid
+ *   pairs_dev   [n_terms, 3] int32 (p, q, interval): the (baseline, interval) combinations that carry
+ *               planned visibilities;  weights_dev [n_terms] float64: their visibility counts;
+ *   weight_sum  the sum of the weights;  avg_dev [L, L] float64, overwritten.
+ * idg_plan_power_norm_terms lists the terms of a plan on the HOST (no GPU needed), in the order
+ * idg_power_norm_average uses, so that both calls return bit-identical averages: call it with capacity 0 to
+ * get n_terms and weight_sum, then with pairs_host [n_terms, 3] / weights_host [n_terms] (capacity =
+ * n_terms; IDG_ENOMEM if too small), and copy both into your own device memory once. */
+#define IDG_STATIC_MAX_SUBGRID_SIZE 96
+IDG_API int  idg_plan_power_norm_terms(const idg_plan* plan, int32_t* pairs_host, double* weights_host,
+                               int64_t capacity, int64_t* n_terms, double* weight_sum);
+IDG_API int  idg_power_norm_average_static(const void* aterms_dev, int32_t subgrid_size, int32_t n_intervals,
+                                   const int32_t* pairs_dev, const double* weights_dev, int64_t n_terms,
+                                   double weight_sum, double* avg_dev, void* cuda_stream);
+
 /* Empirical ALU peaks of the current device, measured the way the paper measures its Table 1
  * (§5.1 :339-351): register-only loops timed with the SM cycle counter.  Synchronous.
  * out_host[7], per SM per clock: [0] FFMA lane-ops, [1] FFMA2 (packed fp32x2) FMA lane-ops,

@@ -27,6 +27,7 @@ SYMBOLS = (
     "idg_grid_subgrids", "idg_degrid_subgrids", "idg_subgrid_fft", "idg_adder", "idg_splitter",
     "idg_closure_workspace_bytes", "idg_grid_to_image", "idg_image_to_grid",
     "idg_grid_subgrids_f64", "idg_degrid_subgrids_f64", "idg_power_norm_average",
+    "idg_plan_power_norm_terms", "idg_power_norm_average_static",
     "idg_profile_enable", "idg_profile_read", "idg_kernel_config_mask", "idg_plan_kernel_split",
     "idg_measure_alu_peaks", "idg_launch_count", "idg_last_error", "idg_version",
 )
@@ -117,6 +118,10 @@ def load_library() -> ctypes.CDLL:
     lib.idg_degrid_subgrids_f64.restype = ctypes.c_int
     lib.idg_power_norm_average.argtypes = [vp, vp, vp, vp]
     lib.idg_power_norm_average.restype = ctypes.c_int
+    lib.idg_plan_power_norm_terms.argtypes = [vp, vp, vp, i64, ctypes.POINTER(i64), ctypes.POINTER(ctypes.c_double)]
+    lib.idg_plan_power_norm_terms.restype = ctypes.c_int
+    lib.idg_power_norm_average_static.argtypes = [vp, ctypes.c_int32, ctypes.c_int32, vp, vp, i64, ctypes.c_double, vp, vp]
+    lib.idg_power_norm_average_static.restype = ctypes.c_int
     lib.idg_measure_alu_peaks.argtypes = [vp]
     lib.idg_measure_alu_peaks.restype = ctypes.c_int
     lib.idg_launch_count.argtypes = []
@@ -274,7 +279,7 @@ def plan_from_config(cfg, uvw_m, freqs, baselines, max_batch_subgrids=0, **kw) -
                 comfort=cfg.comfort, max_batch_subgrids=max_batch_subgrids, **kw)
 
 
-_DTYPES = {"c64": ("complex64",), "c128": ("complex128",), "f32": ("float32",), "f64": ("float64",)}
+_DTYPES = {"c64": ("complex64",), "c128": ("complex128",), "f32": ("float32",), "f64": ("float64",), "i32": ("int32",)}
 
 
 def _expect(t, kind: str, numel: int, what: str, at_least: bool = False) -> None:
@@ -412,6 +417,36 @@ def power_norm_average(plan: Plan, aterms, avg_out, stream=None) -> None:
     _expect(avg_out, "f64", plan.subgrid_size ** 2, "avg [L, L]")
     _check(load_library().idg_power_norm_average(plan.handle, _ptr(aterms), _ptr(avg_out), _stream_ptr(stream)),
            "idg_power_norm_average")
+
+
+def plan_power_norm_terms(plan: Plan):
+    """idg_plan_power_norm_terms (host only): (pairs [n, 3] int32 of (p, q, interval), weights [n] float64,
+    weight_sum) -- the inputs of power_norm_average_static, in the order idg_power_norm_average uses."""
+    lib = load_library()
+    n, wsum = ctypes.c_int64(0), ctypes.c_double(0.0)
+    _check(lib.idg_plan_power_norm_terms(plan.handle, None, None, 0, ctypes.byref(n), ctypes.byref(wsum)),
+           "idg_plan_power_norm_terms")
+    pairs = np.zeros((n.value, 3), np.int32)
+    weights = np.zeros(n.value, np.float64)
+    if n.value:
+        _check(lib.idg_plan_power_norm_terms(plan.handle, pairs.ctypes.data, weights.ctypes.data, n.value,
+                                             ctypes.byref(n), ctypes.byref(wsum)), "idg_plan_power_norm_terms")
+    return pairs, weights, float(wsum.value)
+
+
+def power_norm_average_static(aterms, subgrid_size, n_intervals, pairs, weights, weight_sum, avg_out,
+                              stream=None) -> None:
+    """idg_power_norm_average_static: the average of power_norm_average without any device allocation (scratch
+    built into the library, subgrid_size <= 96, calls on one device must not overlap).  Every array is a CUDA
+    tensor the caller owns: pairs [n, 3] int32, weights [n] float64, avg_out [L, L] float64."""
+    _need_cuda(aterms, pairs, weights, avg_out)
+    n = int(weights.numel())
+    _expect(pairs, "i32", n * 3, "pairs [n_terms, 3]")
+    _expect(weights, "f64", n, "weights [n_terms]")
+    _expect(avg_out, "f64", subgrid_size ** 2, "avg [L, L]")
+    _check(load_library().idg_power_norm_average_static(_ptr(aterms), int(subgrid_size), int(n_intervals), _ptr(pairs),
+                                                        _ptr(weights), n, float(weight_sum), _ptr(avg_out),
+                                                        _stream_ptr(stream)), "idg_power_norm_average_static")
 
 
 def subgrid_fft(subgrid_size, planes, direction, stream=None) -> None:

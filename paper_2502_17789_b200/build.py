@@ -19,7 +19,7 @@ INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libidg_b200.so")
 
-SOURCES = ["plan.cpp", "api.cu", "gridder.cu", "gridder_tc.cu", "degridder.cu", "degridder_tc.cu", "direct_f64.cu", "fft.cu", "adder.cu", "closure.cu", "peaks.cu"]
+SOURCES = ["plan.cpp", "api.cu", "gridder.cu", "gridder_tc.cu", "degridder.cu", "degridder_tc.cu", "direct_f64.cu", "fft.cu", "adder.cu", "closure.cu", "peaks.cu", "no_alloc.cu"]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-ffp-contract=off", "-Xcompiler", "-fvisibility=hidden",
