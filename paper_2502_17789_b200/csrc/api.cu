@@ -536,10 +536,16 @@ void ensure_row_runs(const idg_plan* plan) {
 }
 
 // Calls fn(byte offset, byte count) for the touched rows of every (layer, polarisation) plane of the master grid.
-cudaError_t for_grid_rows(const idg_plan* plan, const std::function<cudaError_t(size_t, size_t)>& fn) {
+// row_align > 1 widens each range outwards to multiples of row_align (clamped to the grid).
+cudaError_t for_grid_rows(const idg_plan* plan, const std::function<cudaError_t(size_t, size_t)>& fn, int row_align = 1) {
   const size_t Ng = plan->par.grid_size;
   for (int32_t k = 0; k < plan->n_wlayers; ++k) {
-    const auto gr = plan->grid_rows[k];
+    auto gr = plan->grid_rows[k];
+    if (gr.second <= gr.first) continue;
+    if (row_align > 1) {
+      gr.first = gr.first / row_align * row_align;
+      gr.second = std::min<int32_t>(plan->par.grid_size, (gr.second + row_align - 1) / row_align * row_align);
+    }
     const size_t n = static_cast<size_t>(gr.second - gr.first) * Ng * sizeof(float2);
     if (n == 0) continue;
     for (int p = 0; p < 4; ++p) {
@@ -659,8 +665,10 @@ int idg_grid_host(const idg_plan* plan, const void* vis_host, const void* aterms
   // The caller's grid (accumulated into) is NOT on the critical path: the subgrids are added into a zeroed
   // device grid while the caller's grid goes up to a second buffer behind the visibilities, and the two are
   // summed once at the end.
-  // (only the rows under a subgrid are zeroed, added and moved: nothing else of the device grid is ever read)
-  IDG_CUDA(for_grid_rows(plan, [&](size_t off, size_t n) { return cudaMemsetAsync(base + a.grid + off, 0, n, stream); }));
+  // (only the rows under a subgrid are added and moved.  The adder reads and writes whole tiles of tile_h rows,
+  // so the zeroed range is widened to tile rows: nothing else of the device grid is ever read.)
+  IDG_CUDA(for_grid_rows(plan, [&](size_t off, size_t n) { return cudaMemsetAsync(base + a.grid + off, 0, n, stream); },
+                         plan->tile_h));
   for (size_t i = 0; i < plan->batches.size(); ++i) {
     for (const auto& run : plan->rows_first[i])
       IDG_CUDA(cudaMemcpyAsync(base + a.vis + run.first * row_b, static_cast<const char*>(vis_host) + run.first * row_b,

@@ -121,8 +121,8 @@ __global__ void __launch_bounds__(T) degridder_kernel(const SubgridJob job, cons
           float2 tt[PV / 2];
 #pragma unroll
           for (int j = 0; j < PV / 2; ++j)
-            tt[j] = make_float2(static_cast<float>(afix[2 * j] * ix0 + bfix[2 * j] * iy) * 1.4629180792671596e-9f,
-                                static_cast<float>(afix[2 * j + 1] * ix0 + bfix[2 * j + 1] * iy) * 1.4629180792671596e-9f);
+            tt[j] = make_float2(static_cast<float>(wrap_dot2(afix[2 * j], ix0, bfix[2 * j], iy)) * 1.4629180792671596e-9f,
+                                static_cast<float>(wrap_dot2(afix[2 * j + 1], ix0, bfix[2 * j + 1], iy)) * 1.4629180792671596e-9f);
 #pragma unroll 2
           for (int i = 0; i < kSeg; ++i) {
             const float4* rec = spix[seg * kSeg + i];

@@ -344,7 +344,7 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
 #ifdef IDG_DTC_FLOATBASE
             const float base = fmaf(al, static_cast<float>(ix0), be_f * static_cast<float>(iy));
 #else
-            const float base = static_cast<float>(alpha_fix * ix0 + beta_fix * iy) * 1.4629180792671596e-9f;   // 2 pi / 2^32
+            const float base = static_cast<float>(wrap_dot2(alpha_fix, ix0, beta_fix, iy)) * 1.4629180792671596e-9f;   // 2 pi / 2^32
 #endif
             const float2 base2 = make_float2(base, base), al2 = make_float2(al, al), ga2 = make_float2(ga, ga);
             const float2 m1 = make_float2(-1.f, -1.f);

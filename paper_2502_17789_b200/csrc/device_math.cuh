@@ -2,6 +2,8 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <cstdint>
+
 namespace idg {
 
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
@@ -45,6 +47,14 @@ __device__ __forceinline__ float frobenius_inv(float4 mp0, float4 mp1, float4 mq
   const float n2 = (p00.x * p00.x + p00.y * p00.y) + (p01.x * p01.x + p01.y * p01.y) +
                    (p10.x * p10.x + p10.y * p10.y) + (p11.x * p11.x + p11.y * p11.y);
   return __fdiv_rn(1.f, __fsqrt_rn(n2));
+}
+
+// a * x + b * y modulo 2^32, as the signed value in [-2^31, 2^31): the fixed-point phase in cycles * 2^32, which is
+// MEANT to wrap (exact modulo one cycle).  The arithmetic is unsigned because signed overflow is undefined
+// behaviour in C++: a compiler may assume it never happens and widen or reorder the products.
+__device__ __forceinline__ int32_t wrap_dot2(int32_t a, int32_t x, int32_t b, int32_t y) {
+  return static_cast<int32_t>(static_cast<uint32_t>(a) * static_cast<uint32_t>(x) +
+                              static_cast<uint32_t>(b) * static_cast<uint32_t>(y));
 }
 
 __device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }

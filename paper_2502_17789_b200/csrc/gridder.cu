@@ -138,12 +138,12 @@ __global__ void __launch_bounds__(T) gridder_kernel(const SubgridJob job, const 
       // per-(row, pixel) slope and offset of the phase; amortised over the row's channels
       const RowData rd = srow[buf];
       const float ax = rd.us * fx;
-      const int32_t bx = rd.alpha_fix * (ix - L / 2);
+      const uint32_t bx = static_cast<uint32_t>(rd.alpha_fix) * static_cast<uint32_t>(ix - L / 2);   // unsigned: meant to wrap
 #pragma unroll
       for (int j = 0; j < P; ++j) {
         const int iy = iy0 + j * YSTEP - L / 2;
         pa[j] = fmaf(rd.vs, static_cast<float>(iy), fmaf(rd.ws, np[j], ax));
-        const int32_t bf = bx + rd.beta_fix * iy;                       // wraps: exact mod 1 cycle
+        const int32_t bf = static_cast<int32_t>(bx + static_cast<uint32_t>(rd.beta_fix) * static_cast<uint32_t>(iy));   // exact mod 1 cycle
         pb[j] = fmaf(rd.gamma, np[j], static_cast<float>(bf) * 1.4629180792671596e-9f);  // 2 pi / 2^32
       }
     }

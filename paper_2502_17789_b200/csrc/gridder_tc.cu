@@ -466,7 +466,7 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
           rd.alpha_fix = __float_as_int(ra.x); rd.beta_fix = __float_as_int(ra.y); rd.gamma = ra.z; rd.us = ra.w;
           rd.vs = rb.x; rd.ws = rb.y; rd.dmax = rb.z;
           pa = fmaf(rd.vs, static_cast<float>(iy), fmaf(rd.ws, np, rd.us * static_cast<float>(ix)));
-          const int32_t bf = rd.alpha_fix * ix + rd.beta_fix * iy;                  // wraps: exact mod 1 cycle
+          const int32_t bf = wrap_dot2(rd.alpha_fix, ix, rd.beta_fix, iy);                  // wraps: exact mod 1 cycle
           pb = fmaf(rd.gamma, np, static_cast<float>(bf) * 1.4629180792671596e-9f);   // 2 pi / 2^32
           if constexpr (ROT) {
             const float delta = pa * job.dkappa_f;
@@ -495,9 +495,12 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
               sg = 2.f * s2 * (1.f - k2);
               kh = 2.f * s2 * s2;
             } else {
-              float c;
-              sincosf(delta, &sg, &c);
-              kh = 1.f - c;
+              // from the half angle: 1 - cos(delta) would cancel for the pixels near the subgrid centre, whose delta
+              // is small although the row's dmax is not (3e-8 absolute in kh grows as j^2 along the recurrence)
+              float sh, ch;
+              sincosf(0.5f * delta, &sh, &ch);
+              kh = 2.f * sh * sh;
+              sg = 2.f * sh * ch;
             }
             nk2 = make_float2(-2.f * kh, -2.f * kh);
           }
@@ -653,8 +656,11 @@ cudaError_t launch_rot(const SubgridJob& job, const float4* vis, float2* out, cu
   const int cap_chunks = std::min(job.max_nt * cpr_max, kMaxBBytes / CHUNK_BYTES);
   const size_t dyn = static_cast<size_t>(cap_chunks + NA - 1) * CHUNK_BYTES;   // + padding chunks
   auto kernel = gridder_tc_kernel<L, NG, KC, DG, NA, ROT>;
-  // per launch: the attribute belongs to the (function, device) pair and the call is cheap
-  cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(dyn));
+  // per launch (the attribute belongs to the (function, device) pair and the call is cheap), but always the
+  // instantiation's MAXIMUM, never this launch's own size: two host threads with plans of different shapes could
+  // otherwise interleave set(large), set(small), launch(large) and fail the launch
+  constexpr int kDynMax = kMaxBBytes + (NA - 1) * CHUNK_BYTES;
+  cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kDynMax);
   if (e != cudaSuccess) return e;
   kernel<<<static_cast<unsigned>(job.count), NG * kTileM + NG * 32, dyn, stream>>>(job, vis, out, cap_chunks);
   count_launch();
@@ -694,12 +700,14 @@ cudaError_t launch_l(const SubgridJob& job, const float4* vis, float2* out, cuda
 
 }  // namespace
 
+bool gridder_tc_fits(int n_chan, int max_nt) {
+  constexpr int KC = IDG_TC_KC;
+  return n_chan <= kMaxChanTc - KC && max_nt <= kMaxRowsTc && (n_chan + KC - 1) / KC <= kMaxBBytes / (KC * kVisBytes);
+}
+
 cudaError_t launch_gridder_tc(const SubgridJob& job, const float4* vis, float2* out, cudaStream_t stream) {
   // shapes whose per-subgrid constants do not fit the kernel's shared-memory tables take the SIMT kernel
-  constexpr int KC = IDG_TC_KC;
-  if (job.n_chan > kMaxChanTc - KC || job.max_nt > kMaxRowsTc ||
-      (job.n_chan + KC - 1) / KC > kMaxBBytes / (KC * kVisBytes))
-    return launch_gridder(job, vis, out, stream);
+  if (!gridder_tc_fits(job.n_chan, job.max_nt)) return launch_gridder(job, vis, out, stream);
   switch (job.subgrid_size) {
     case 32:  return launch_l<32>(job, vis, out, stream);
     case 48:  return launch_l<48>(job, vis, out, stream);

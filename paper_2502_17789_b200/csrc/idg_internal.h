@@ -120,5 +120,8 @@ void build_tile_csr(const idg_plan* plan, int64_t first, int64_t count, TileCsr*
 void fill_meta(const idg_plan* plan, std::vector<int32_t>* meta);
 bool subgrid_conjugated(const idg_plan* plan, const int32_t* sub8);
 void split_kernels(const idg_plan* plan, int64_t first, int64_t count, int direction, KernelSplit* out);
+// whether the tensor-core gridder's shared-memory tables hold a plan of this shape (gridder_tc.cu); if not, a
+// launch handed to it runs the SIMT kernel, and split_kernels reports it so
+bool gridder_tc_fits(int n_chan, int max_nt);
 
 }  // namespace idg

@@ -235,6 +235,10 @@ bool subgrid_conjugated(const idg_plan* plan, const int32_t* e) {
 void split_kernels(const idg_plan* plan, int64_t first, int64_t count, int direction, KernelSplit* out) {
   out->tensor.clear(); out->simt.clear();
   out->variant = direction == IDG_GRID ? plan->par.gridder_variant : plan->par.degridder_variant;
+  const int32_t max_nt = std::min(plan->par.n_times, plan->par.aterm_period);
+  if (direction == IDG_GRID && out->variant != IDG_VARIANT_SIMT && out->variant != IDG_VARIANT_FP64 &&
+      !gridder_tc_fits(plan->par.n_chan, max_nt))
+    out->variant = IDG_VARIANT_SIMT;      // what launch_gridder_tc would run anyway: the reported split says so
   if (out->variant != IDG_VARIANT_AUTO) return;
   for (int64_t i = 0; i < count; ++i) {
     const int32_t* e = &plan->sub[static_cast<size_t>(first + i) * 8];

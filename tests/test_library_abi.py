@@ -122,6 +122,13 @@ def test_kernel_choice_per_subgrid(idg):
         o = synth.make_observation(c, vis=None, with_aterms=False)
         nt, ns = _plan(idg, c, o).kernel_split(idg.IDG_GRID)
         assert (ns == 0) if all_tc else (nt == 0)
+    # a shape whose tables the tensor-core gridder cannot hold (1300 channels > 1264) runs the SIMT kernel whatever
+    # was asked for, and the split says so (what launches is what is reported)
+    c = synth.scaled(synth.get_config(1), n_stations=3, n_times=4, n_chan=1300, chan_width_hz=150.0)
+    o = synth.make_observation(c, vis=None, with_aterms=False)
+    for v in (idg.VARIANT_AUTO, idg.VARIANT_TENSOR):
+        p = _plan(idg, c, o, gridder_variant=v)
+        assert p.kernel_split(idg.IDG_GRID) == (0, p.counts().n_subgrids)
 
 
 def test_workspace_follows_batch_capacity(idg):
