@@ -123,7 +123,10 @@ IDG_API int  idg_grid(const idg_plan* plan, const void* vis_dev, const void* ate
 
 /* The same with imaging weights applied as the visibilities are loaded ("weighting ...
  * performed by each thread"): vis[r, c, :] is multiplied by weights_dev[r, c]
- * (float32 [n_rows, n_chan]; NULL = idg_grid).  Flagged samples are weight 0. */
+ * (float32 [n_rows, n_chan]; NULL = idg_grid).  Flagged samples are weight 0: such a sample contributes an exact
+ * zero whatever it holds (NaN and Inf included; it is selected out, not multiplied) and does not enter the
+ * tensor-core gridder's per-segment scale.  A non-finite sample with a non-zero weight is the caller's error: the
+ * result of every subgrid that covers it is undefined (NaN in its pixels). */
 IDG_API int  idg_grid_weighted(const idg_plan* plan, const void* vis_dev, const float* weights_dev,
                        const void* aterms_dev, const float* taper_dev, void* grid_dev, void* workspace_dev,
                        size_t workspace_bytes, void* cuda_stream);

@@ -107,7 +107,8 @@ __global__ void __launch_bounds__(kT) gridder_f64_kernel(const SubgridJob job, c
         }
 #pragma unroll
         for (int p = 0; p < 4; ++p) {
-          const double re = x[p].x * wgt, im = x[p].y * wgt;
+          // weight 0 = flagged: an exact zero whatever the sample holds
+          const double re = wgt == 0.0 ? 0.0 : x[p].x * wgt, im = wgt == 0.0 ? 0.0 : x[p].y * wgt;
           acc[p].x += re * cs - im * sn;
           acc[p].y += re * sn + im * cs;
         }

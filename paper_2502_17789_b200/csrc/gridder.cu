@@ -91,7 +91,8 @@ __global__ void __launch_bounds__(T) gridder_kernel(const SubgridJob job, const 
       }
       if (job.weights != nullptr) {                     // weighting at load
         const float wgt = __ldg(&job.weights[(row0 + r) * job.n_chan + c0 + cc + (tid >> 1)]);
-        pre = make_float4(pre.x * wgt, pre.y * wgt, pre.z * wgt, pre.w * wgt);
+        // weight 0 = flagged: an exact zero whatever the sample holds (NaN * 0 would poison the pixel sums)
+        pre = wgt == 0.f ? make_float4(0.f, 0.f, 0.f, 0.f) : make_float4(pre.x * wgt, pre.y * wgt, pre.z * wgt, pre.w * wgt);
       }
     }
   };

@@ -277,7 +277,7 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
           float2 v = load_vis(r, cc + j, p);
           if (job.weights != nullptr) {
             const float wgt = __ldg(&job.weights[(row0 + r) * job.n_chan + c0 + cc + j]);
-            v = make_float2(v.x * wgt, v.y * wgt);
+            v = wgt == 0.f ? make_float2(0.f, 0.f) : make_float2(v.x * wgt, v.y * wgt);   // flagged: out of the scale too
           }
           mx = fmaxf(mx, fmaxf(fabsf(v.x), fabsf(v.y)));
         }
@@ -299,7 +299,7 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
         v = load_vis(r, cc + j, p);
         if (job.weights != nullptr) {
           const float wgt = __ldg(&job.weights[(row0 + r) * job.n_chan + c0 + cc + j]);
-          v = make_float2(v.x * wgt, v.y * wgt);
+          v = wgt == 0.f ? make_float2(0.f, 0.f) : make_float2(v.x * wgt, v.y * wgt);   // weight 0 = flagged: exact zero
         }
         v = make_float2(v.x * vinv, v.y * vinv);
       }
@@ -326,7 +326,7 @@ __global__ void __launch_bounds__(NG* kTileM + NG * 32, NG == 1 ? 4 : (NG == 2 ?
         v = load_vis(r, cc + j, p);
         if (job.weights != nullptr) {                  // weighting at load
           const float wgt = __ldg(&job.weights[(row0 + r) * job.n_chan + c0 + cc + j]);
-          v = make_float2(v.x * wgt, v.y * wgt);
+          v = wgt == 0.f ? make_float2(0.f, 0.f) : make_float2(v.x * wgt, v.y * wgt);   // weight 0 = flagged: exact zero
         }
       }
       const float hr = tf32_round(v.x), hi = tf32_round(v.y);

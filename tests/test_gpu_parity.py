@@ -10,7 +10,7 @@ import torch
 
 import synth
 from oracle import idg_oracle as orc
-from tests.util import inner, oracle_params, random_jones
+from tests.util import check_gridder_subgrids, inner, oracle_params, random_jones
 
 pytestmark = pytest.mark.gpu
 
@@ -443,12 +443,20 @@ def test_full_size_config2_sampled(idg):
     d_vis, d_at, d_tp = dev(obs.vis), dev(obs.aterms), dev(obs.taper)
     d_grid = torch.zeros((cnt.n_wlayers, 4, Ng, Ng), dtype=torch.complex64, device=DEV)
     ws = torch.empty(plan.workspace_bytes(), dtype=torch.uint8, device=DEV)
+    idg.kernel_config_mask("gridder", reset=True)
     idg.grid(plan, d_vis, d_at, d_tp, d_grid, ws)
+    mask_full = idg.kernel_config_mask("gridder")
     d_grid2 = torch.zeros_like(d_grid)
     idg.grid(plan, d_vis, d_at, d_tp, d_grid2, ws)
     assert torch.equal(torch.view_as_real(d_grid), torch.view_as_real(d_grid2)), "not bitwise reproducible"
     del d_grid2
     g = d_grid.cpu().numpy()
+
+    # --- per subgrid (north_star's metric for the imaging direction), in windows of the full plan that run the
+    # launch configuration the whole batch runs
+    w_s, w_f, mask_win = check_gridder_subgrids(idg, plan, par, obs, sub, obs.vis, d_vis, d_at, d_tp,
+                                                sample_subgrids(sub, 8, seed=12))
+    assert mask_win == mask_full and not mask_full & idg.KMASK_SIMT, (mask_win, mask_full)
 
     # --- grid pixels covered by few subgrids (the outskirts of the uv coverage)
     x0, y0 = sub[:, 5].astype(np.int64), sub[:, 6].astype(np.int64)
@@ -462,13 +470,21 @@ def test_full_size_config2_sampled(idg):
     cands.sort(key=lambda c: c[0])
     picks = cands[:4] + cands[len(cands) // 8: len(cands) // 8 + 2]     # the sparsest and two busier pixels
     assert picks[-1][0] <= 400, "sampled pixels are too expensive for the oracle"
+    w_pix = w_pix_g = 0.0
     for _, py, px, cover in picks:
         want = np.zeros(4, np.complex128)
+        local = 0.0                                   # the largest value of any subgrid that covers the pixel
         for c in cover:
             _, Shat = orc.grid_subgrid(par, sub[c], obs.uvw, obs.freqs, obs.vis, obs.baselines, obs.aterms, obs.taper)
             want += Shat[py - y0[c], px - x0[c], :]
+            local = max(local, float(np.abs(Shat).max()))
         got = g[0, :, py, px]
-        assert np.abs(got - want).max() <= TOL * max(scale, np.abs(want).max()), (py, px, cover.tolist(), got, want)
+        # normalised by the covering subgrids' maximum, not by the dense core's (`scale`, 10^2-10^3 larger)
+        assert np.abs(got - want).max() <= TOL * local, (py, px, cover.tolist(), got, want, local)
+        w_pix = max(w_pix, np.abs(got - want).max() / local)
+        w_pix_g = max(w_pix_g, np.abs(got - want).max() / max(scale, np.abs(want).max()))
+    print(f"config 2 full size: worst per-subgrid error {w_s:.2e} after the gridder, {w_f:.2e} after the FFT; worst "
+          f"grid-pixel error {w_pix:.2e} of the covering subgrids' maximum ({w_pix_g:.2e} of the grid's)")
 
     # --- prediction of sampled subgrids from this grid
     d_out = torch.full((cfg.n_rows, cfg.n_chan, 4), float("nan"), dtype=torch.complex64, device=DEV)
@@ -484,7 +500,7 @@ def test_full_size_config2_sampled(idg):
         assert e <= TOL, (s, sub[s].tolist(), e)
 
 
-@pytest.mark.parametrize("variant", ["simt", "tensor"])
+@pytest.mark.parametrize("variant", ["simt", "tensor", "fp64"])
 def test_weighted_gridding(idg, variant):
     """SURVEY §8(f) NEXT-2, weights at load: idg_grid_weighted == the oracle on vis * weights,
     zero weights (flags) included."""
@@ -501,6 +517,18 @@ def test_weighted_gridding(idg, variant):
     ref = orc.grid(par, sub, obs.uvw, obs.freqs, obs.vis.astype(np.complex128) * wgt[:, :, None].astype(np.float64),
                    obs.baselines, obs.aterms, obs.taper)
     assert nerr(d_grid.cpu().numpy(), ref) <= TOL
+    # flagged samples of real measurement sets hold NaN (or anything): weight 0 must select them out, not multiply
+    # them (NaN * 0 = NaN would poison the pixel sums, and the tensor-core gridder's segment scale with them)
+    junk = obs.vis.copy()
+    flagged = wgt == 0.0
+    fill = np.array([np.nan, np.inf, -np.inf, 3e38], np.float32)[rng.integers(0, 4, int(flagged.sum()))]
+    junk[flagged] = (fill + 1j * fill[::-1])[:, None]
+    assert not np.isfinite(junk).all()
+    d_grid.zero_()
+    idg.grid_weighted(plan, dev(junk), dev(wgt), dev(obs.aterms), dev(obs.taper), d_grid, ws)
+    got = d_grid.cpu().numpy()
+    assert np.isfinite(got).all(), "a flagged sample leaked into the grid"
+    assert nerr(got, ref) <= TOL
 
 
 def test_tensor_gridder_dynamic_range(idg):

@@ -57,3 +57,29 @@ def device_inner(a, b, chunk=1 << 24):
         y = fb[i:i + chunk].to(torch.complex128)
         acc += complex(torch.sum(torch.conj(x) * y).item())
     return acc
+
+
+def check_gridder_subgrids(idg, plan, par, obs, sub, vis, d_vis, d_at, d_tp, picks, window=64, tol=1e-5):
+    """north_star's metric for the imaging direction, usable at any size: subgrid s after the gridder + A-term + taper
+    (steps a1-a3, Eq. 10) and after the subgrid FFT (a4, :157) against the oracle's subgrid,
+    max |gpu - oracle| / max |oracle| of THAT subgrid <= tol.  Each pick is computed inside a window of neighbouring
+    subgrids through idg_grid_subgrids, i.e. with the plan's own kernel choice and launch configuration.
+    `vis` is what the oracle slices (numpy array or OnDevice).  Returns (worst after a3, worst after a4, the
+    gridder kernel mask of the windows)."""
+    import torch
+    L, n = par.subgrid_size, len(sub)
+    worst = [0.0, 0.0]
+    idg.kernel_config_mask("gridder", reset=True)
+    for s in picks:
+        first = min(max(0, s - window // 2), max(0, n - window))
+        count = min(window, n - first)
+        Sp, Shat = orc.grid_subgrid(par, sub[s], obs.uvw, obs.freqs, vis, obs.baselines, obs.aterms, obs.taper)
+        out = torch.empty((count, 4, L, L), dtype=torch.complex64, device=d_vis.device)
+        for k, (stage, want) in enumerate(((idg.STAGE_GRIDDER, Sp), (idg.STAGE_FFT, Shat))):
+            out.fill_(float("nan"))
+            idg.grid_subgrids(plan, first, count, d_vis, d_at, d_tp, out, stage=stage)
+            got = np.moveaxis(out[s - first].cpu().numpy(), 0, 2)
+            e = float(np.abs(got - want).max() / np.abs(want).max())
+            assert e <= tol, (int(s), sub[s].tolist(), "gridder" if k == 0 else "fft", e)
+            worst[k] = max(worst[k], e)
+    return worst[0], worst[1], idg.kernel_config_mask("gridder", reset=True)
