@@ -307,6 +307,33 @@ def kernel_rooflines(cfg, sub, n_wlayers, prof_ms, prof_n, steps, peaks, sm_mhz_
     return out, peak_tflops, flop, alg_bytes
 
 
+# What binds the tensor-core direct sums, beside the survey's SIMT roofline (18 FP32-pipe ops per pair, which charges
+# the 16 MACs to the FP32 pipe although they run on the tensor pipe, so the gridder can exceed it).  Per (visibility,
+# pixel) pair: MUFU operations the shipped kernel issues (rotating gridder: one __sincosf per 8 channels = 0.25;
+# degridder: one per pair = 2) and warp instructions ISSUED per pair as ncu counted them in the committed capture
+# (profiles/ncu_r03_summary.md: smsp__inst_executed.sum x 32 / pairs).  Peaks per SM clock: 16 SFU lanes
+# (MUFU.EX2 measured 16.0, profiles/alu_peaks_r01.md), 4 schedulers x 32 lanes = 128 issued thread-instructions.
+CEILING_INPUTS = {"gridder": {"mufu_per_pair": 0.25, "issued_per_pair": 12.4},
+                  "degridder": {"mufu_per_pair": 2.0, "issued_per_pair": 14.8}}
+SFU_LANES_PER_SM, ISSUE_LANES_PER_SM = 16.0, 128.0
+
+
+def ceilings(kernel, pairs_per_clk_per_sm):
+    """Ceilings of a tensor-core direct-sum kernel in pairs per SM clock, and the fraction of the tightest one that
+    is a true bound for it (the SIMT-equivalent FP32 figure is kept as a label, not as a bound)."""
+    c = CEILING_INPUTS[kernel]
+    sfu = SFU_LANES_PER_SM / c["mufu_per_pair"]
+    issue = ISSUE_LANES_PER_SM / c["issued_per_pair"]
+    out = {"unit": "pairs/clk/SM", "simt_equivalent_fp32": FP32_LANES_PER_SM / FP32_OPS_PER_PAIR, "sfu": sfu,
+           "issue_slots": issue, "mufu_per_pair": c["mufu_per_pair"], "issued_instructions_per_pair": c["issued_per_pair"],
+           "source": "profiles/ncu_r03_summary.md (instructions per pair), profiles/alu_peaks_r01.md (pipe widths)",
+           "binding": "sfu" if sfu < issue else "issue_slots"}
+    if pairs_per_clk_per_sm:
+        out["achieved"] = pairs_per_clk_per_sm
+        out["frac_of_binding"] = pairs_per_clk_per_sm / min(sfu, issue)
+    return out
+
+
 VARIANTS = {"auto": 0, "simt": 1, "tensor": 2, "fp64": 3}      # IDG_VARIANT_* of include/idg_b200.h
 OPERANDS = ("direct sums on tcgen05: gridder fp16 head + fp16 remainder of (cos, sin) and of the visibilities (one "
             "power-of-two scale per segment), degridder tf32 head + tf32 remainder; fp32 accumulation in tensor memory, "
@@ -372,7 +399,8 @@ def device_leg(idg, torch, cfg, plan, sub, cnt, d_vis, d_at, d_tp, steps, warmup
 
 
 def other_config(idg, torch, config_id, dev, stream, barrier, peaks, sampler_index):
-    """One warm-up and two timed steps of another BASELINE.json config (3, 4: grid + degrid; 5: prediction only, from
+    """One warm-up and two timed steps of another BASELINE.json config (1, 3, 4: grid + degrid; config 1 is 56 subgrids
+    of 32 visibilities, launch-latency-bound: reported, not tuned for; 5: prediction only, from
     the grid of one imaging pass), visibilities by the counter-based hash recipe generated on the device (the
     values do not affect timing).  The headline `value`, `config` and `roofline` stay config 2's."""
     cfg = synth.get_config(config_id)
@@ -504,7 +532,7 @@ def run_ours(args):
     others = None
     if rank == 0 and world == 1 and cfg.config_id == 2 and not args.no_other_configs:
         others = {}
-        for c in (3, 4, 5):
+        for c in (1, 3, 4, 5):
             others[str(c)] = other_config(idg, torch, c, dev, stream, barrier, peaks, torch.cuda.current_device())
 
     if rank != 0:
@@ -520,7 +548,13 @@ def run_ours(args):
                 "peak_basis": f"{N_SM} SM x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {peaks['sm_max_mhz']:.0f} MHz "
                               f"(sm_max_mhz {peaks['source']}); work = 18 FP32-pipe ops per (vis,pixel) pair",
                 "frac_at_observed_clock": kr[dom]["frac_at_observed_clock"],
-                "hbm_frac_of_measured": kr[dom]["hbm_frac"], "hbm_peak_gbs": peaks["hbm_gbs"]}
+                "hbm_frac_of_measured": kr[dom]["hbm_frac"], "hbm_peak_gbs": peaks["hbm_gbs"],
+                # `frac` is the survey's SIMT roofline; what actually binds the tensor-core kernels, per kernel:
+                "ceilings": {k: ceilings(k, kr[k].get("pairs_per_clk_per_sm")) for k in cands
+                             if getattr(args, k + "_variant") in ("auto", "tensor")},
+                # every kernel of the headline config (the stored record keeps `roofline`)
+                "per_kernel": {k: {"ms_per_step": v["ms_per_step"], "bound": v["bound"], "frac": v["frac"]}
+                               for k, v in kr.items()}}
     metric = METRIC if not prediction_only else "degridded (predicted) visibilities/s (4 pols each)"
     line = {"metric": metric, "value": value, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": warmup, "ms_per_step": ms_per_step,
@@ -539,7 +573,7 @@ def run_ours(args):
 def ncu_traffic(kernel, cfg, n_subgrids, launches_per_step):
     """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/), scaled from the
     captured launch to this run's average launch; None when there is no capture for this workload."""
-    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "dram_traffic_r02c.csv")
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "dram_traffic_r03a.csv")
     if cfg.config_id != 2 or not os.path.exists(path) or not launches_per_step:
         return None
     with open(path) as f:
