@@ -241,16 +241,18 @@ IDG_API int  idg_image_to_grid(const idg_plan* plan, const void* image_dev, cons
 #define IDG_VARIANT_TENSOR 2
 #define IDG_VARIANT_FP64   3
 
+/* How IDG_VARIANT_AUTO splits the plan's subgrids between the tensor-core and the SIMT kernel of a direction
+ * (IDG_GRID or IDG_DEGRID), summed over the batches.  A plan with a forced variant reports all subgrids under it
+ * (FP64 counts as SIMT); a shape whose per-subgrid tables the tensor-core gridder cannot hold in shared memory (more
+ * than 1264 channels, more than 128 rows per A-term interval) runs the SIMT gridder whatever was asked for and is
+ * reported so.  Host only. */
+IDG_API int  idg_plan_kernel_split(const idg_plan* plan, int direction, int64_t* n_tensor, int64_t* n_simt);
+
 /* Which kernels the direct-sum step `kind` (IDG_K_GRIDDER or IDG_K_DEGRIDDER) has launched in this process
  * since the last reset, as a bit mask: bit 0 SIMT, bit 1 / 2 / 4 tensor-core with 1 / 2 / 4 compute groups
  * per CTA (the gridder picks by shared-memory fit; the degridder always runs 2), bit 8 fp64, bit 9 the tensor-core
  * gridder with phasor rotation along the channel axis (uniformly spaced channels; otherwise one sincos per pair).  reset != 0
  * clears the mask after reading.  For the tests, which must know what they exercised. */
-/* How IDG_VARIANT_AUTO splits the plan's subgrids between the tensor-core and the SIMT kernel of a direction
- * (IDG_GRID or IDG_DEGRID), summed over the batches.  A plan with a forced variant reports all subgrids under it
- * (FP64 counts as SIMT).  Host only. */
-IDG_API int  idg_plan_kernel_split(const idg_plan* plan, int direction, int64_t* n_tensor, int64_t* n_simt);
-
 #define IDG_KMASK_SIMT   (1 << 0)
 #define IDG_KMASK_TC(ng) (1 << (ng))
 #define IDG_KMASK_FP64   (1 << 8)

@@ -48,8 +48,8 @@ def is_stale() -> bool:
     return any(os.path.getmtime(d) > t for d in _deps())
 
 
-def _compile(src: str, verbose: bool, extra=(), tag: str = "") -> str:
-    obj = os.path.join(BUILD, os.path.splitext(src)[0] + tag + ".o")
+def _compile(src: str, verbose: bool, extra=(), tag: str = "", objdir: str = BUILD) -> str:
+    obj = os.path.join(objdir, os.path.splitext(src)[0] + tag + ".o")
     cmd = [_nvcc(), *NVCC_FLAGS, *extra, "-c", os.path.join(CSRC, src), "-o", obj]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
@@ -63,14 +63,16 @@ def _compile(src: str, verbose: bool, extra=(), tag: str = "") -> str:
 
 def build(force: bool = False, verbose: bool = False, extra_flags=(), out: str | None = None) -> str:
     """Compile if needed; returns the path of the shared library.  `extra_flags` / `out` build a
-    differently configured copy (e.g. -D tuning macros) next to the default one."""
+    differently configured copy (e.g. -D tuning macros); its object files go beside `out`, not into the
+    in-tree build directory (which every gpurun call ships to the GPU box)."""
     lib = out or LIB
     if out is None and not force and not is_stale():
         return LIB
-    os.makedirs(BUILD, exist_ok=True)
+    objdir = BUILD if out is None else os.path.dirname(os.path.abspath(out))
+    os.makedirs(objdir, exist_ok=True)
     tag = "" if out is None else "." + os.path.splitext(os.path.basename(out))[0]
     with concurrent.futures.ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
-        objs = list(ex.map(lambda s: _compile(s, verbose, tuple(extra_flags), tag), SOURCES))
+        objs = list(ex.map(lambda s: _compile(s, verbose, tuple(extra_flags), tag, objdir), SOURCES))
     cmd = [_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", lib, *objs,
            "-lcufft", "-Xlinker", "-rpath=/usr/local/cuda/lib64"]     # cuFFT: master-grid FFT of the closure only
     r = subprocess.run(cmd, capture_output=True, text=True)

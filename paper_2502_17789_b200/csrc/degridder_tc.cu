@@ -157,9 +157,6 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
         const int gst = sc0 + st, slot = gst & (NS - 1);
         if (gst >= NS) tc::mbar_wait_backoff(bar_sempty + 8 * slot, ((gst / NS) - 1) & 1, 256);
         float* Bs = reinterpret_cast<float*>(sB + slot * kStageBBytes);
-#ifdef IDG_DTC_FAKE_PRODUCER
-        if (gst < NS)
-#endif
 #pragma unroll 2
         for (int i = 0; i < kStagePix / (32 * kProducers); ++i) {
           const int lp = (pw * (kStagePix / (32 * kProducers)) + i) * 32 + lane, pix = st * kStagePix + lp;
@@ -258,7 +255,6 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
       // fp32 resolves to 1e-6, so a chunk's first pixel takes it modulo one cycle EXACTLY, in 32-bit fixed
       // point (alpha_fix * ix + beta_fix * iy wraps), as the gridders do; only al * j (j < 8) and ga n' are fp32.
       float al = 0.f, ga = 0.f;
-      [[maybe_unused]] float be_f = 0.f;
       int32_t alpha_fix = 0, beta_fix = 0;             // cycles per pixel * 2^32
       if (vis_ok) {
         const double S = job.image_size;
@@ -271,9 +267,6 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
         const double sgn = conj ? -1.0 : 1.0;
         const double alpha = (sgn * uvw[0] * kap - u0) * (S / L), beta = (sgn * uvw[1] * kap - v0) * (S / L);
         al = static_cast<float>(two_pi * alpha);
-#ifdef IDG_DTC_FLOATBASE
-        be_f = static_cast<float>(two_pi * beta);
-#endif
         alpha_fix = static_cast<int32_t>(static_cast<uint32_t>(static_cast<int64_t>(rint(alpha * 4294967296.0))));
         beta_fix = static_cast<int32_t>(static_cast<uint32_t>(static_cast<int64_t>(rint(beta * 4294967296.0))));
         ga = static_cast<float>(two_pi * (sgn * uvw[2] * kap - w0));
@@ -282,11 +275,7 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
       // phasors and stores nothing: it only keeps the ring's barriers in step (its tensor-memory rows hold
       // stale finite-or-not values that no thread reads: MMA rows are independent).  The SIMT work is thus
       // padded to 32 visibilities, not 128 (low-occupancy tails).
-#ifdef IDG_DTC_NOTAIL
-      const bool warp_on = true;
-#else
       const bool warp_on = (t_base + tile_l) * kTileV + (uwarp & 3) * 32 < K;      // from warp-uniform values only
-#endif
       bool pending = false;                            // the ring's last slot is stored but not yet handed over
       auto drain = [&](int qq) {
         tc::mbar_wait(gbar + 16 * NA + 8 * (qq & 1), (qq >> 1) & 1);
@@ -341,11 +330,7 @@ __global__ void __launch_bounds__(NG* kTileV + NG * 32 + kProducers * 32, NG == 
             const float4 na = tc::lds128(np_addr), nb = tc::lds128(np_addr + 16);
             const float2 np2[4] = {make_float2(na.x, na.y), make_float2(na.z, na.w),
                                    make_float2(nb.x, nb.y), make_float2(nb.z, nb.w)};
-#ifdef IDG_DTC_FLOATBASE
-            const float base = fmaf(al, static_cast<float>(ix0), be_f * static_cast<float>(iy));
-#else
             const float base = static_cast<float>(wrap_dot2(alpha_fix, ix0, beta_fix, iy)) * 1.4629180792671596e-9f;   // 2 pi / 2^32
-#endif
             const float2 base2 = make_float2(base, base), al2 = make_float2(al, al), ga2 = make_float2(ga, ga);
             const float2 m1 = make_float2(-1.f, -1.f);
 #pragma unroll

@@ -671,7 +671,7 @@ cudaError_t launch_rot(const SubgridJob& job, const float4* vis, float2* out, cu
 // Rotation along the channel axis needs uniformly spaced channels (job.dkappa != 0, checked by the planner).
 template <int L, int NG, int KC, int DG, int NA>
 cudaError_t launch(const SubgridJob& job, const float4* vis, float2* out, cudaStream_t stream) {
-#if defined(IDG_TC_FP16) && !defined(IDG_TC_NOROT)
+#if defined(IDG_TC_FP16)
   if (job.dkappa != 0.0) return launch_rot<L, NG, KC, DG, NA, true>(job, vis, out, stream);
 #endif
   return launch_rot<L, NG, KC, DG, NA, false>(job, vis, out, stream);
@@ -687,15 +687,11 @@ cudaError_t launch_l(const SubgridJob& job, const float4* vis, float2* out, cuda
   const size_t dyn = static_cast<size_t>(std::min(job.max_nt * ((job.n_chan + KC - 1) / KC), kMaxBBytes / (KC * kVisBytes)) + IDG_TC_NA - 1) *
                      (KC * kVisBytes);
   constexpr size_t kStaticAndReserved = 12 * 1024, kSmemPerSm = 227 * 1024;
-#ifdef IDG_TC_NG
-  return launch<L, IDG_TC_NG, KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
-#else
   if (4 * (dyn + kStaticAndReserved) <= kSmemPerSm) return launch<L, 1, KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
   if (2 * (dyn + kStaticAndReserved) <= kSmemPerSm || ((L * L) / kTileM) % 4 != 0)     // L = 48: 18 tiles
     return launch<L, 2, KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
   if constexpr (((L * L) / kTileM) % 4 == 0) return launch<L, 4, KC, IDG_TC_DG, IDG_TC_NA>(job, vis, out, stream);
   return cudaErrorInvalidValue;
-#endif
 }
 
 }  // namespace
